@@ -1,0 +1,109 @@
+"""ctypes wrapper around the ORACLE (oracle/ark_oracle.cpp).
+
+Test infrastructure only: imported by tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs.  It does not import, and is
+not imported by, the CUDA package paper_1903_09043_b200.
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+BC_PERIODIC, BC_REFLECTING, BC_FIXED_T = 0, 1, 2
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        common = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp, C.c_double, C.c_double,
+                  C.c_int, _ip, _dp]
+        _lib.oracle_run.argtypes = common + [_dp] * 5 + [C.c_int, C.c_double, _dp, _dp, C.c_int]
+        _lib.oracle_run.restype = C.c_int
+        _lib.oracle_max_rate.argtypes = common + [_dp] * 5
+        _lib.oracle_max_rate.restype = C.c_double
+        _lib.oracle_fill_ghosts.argtypes = common + [_dp] * 10
+        _lib.oracle_fill_ghosts.restype = C.c_int
+        _lib.oracle_face.argtypes = [C.c_double] * 8 + [C.c_int, _dp]
+        _lib.oracle_face.restype = None
+        _lib.oracle_K.restype = C.c_double
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _common(p):
+    """p: dict with nx, ny, nz, dx, gamma, g(3), mu, kappa, theta, bc_type(3x2), bc_value(3x2)."""
+    g = np.ascontiguousarray(p["g"], dtype=np.float64)
+    bt = np.ascontiguousarray(np.asarray(p["bc_type"], dtype=np.int32).reshape(6))
+    bv = np.ascontiguousarray(np.asarray(p.get("bc_value", np.zeros((3, 2))), dtype=np.float64).reshape(6))
+    args = [int(p["nx"]), int(p["ny"]), int(p["nz"]), float(p["dx"]), float(p["gamma"]), _ptr(g),
+            float(p["mu"]), float(p["kappa"]), int(p["theta"]), bt.ctypes.data_as(_ip), _ptr(bv)]
+    return args, (g, bt, bv)
+
+
+def _state(p, U):
+    n = int(p["nx"]) * int(p["ny"]) * int(p["nz"])
+    out = []
+    for f in range(5):
+        if f == 3 and int(p["nz"]) == 1 and (len(U) < 5 or U[3] is None):
+            out.append(np.zeros(n))
+            continue
+        a = np.array(U[f], dtype=np.float64, order="C").reshape(-1)
+        assert a.size == n, (a.size, n)
+        out.append(a)
+    return out
+
+
+def run(p, U, nsteps, cfl=None, dts=None, form=0):
+    """Advance a copy of U = [rho, rhou, rhov, rhow, E] (dense, any shape of nx*ny*nz elements,
+    x fastest) by nsteps.  Either dts (array of nsteps prescribed steps) or cfl.  Returns
+    (U_new list of flat arrays, dts_used)."""
+    args, keep = _common(p)
+    S = _state(p, U)
+    dts_in = None if dts is None else np.ascontiguousarray(dts, dtype=np.float64)
+    dts_out = np.zeros(max(nsteps, 1))
+    rc = lib().oracle_run(*args, *[_ptr(a) for a in S], int(nsteps),
+                          float(cfl if cfl is not None else 0.0), _ptr(dts_in), _ptr(dts_out), int(form))
+    if rc != 0:
+        raise FloatingPointError("oracle: non-finite CFL rate (rc=%d)" % rc)
+    return S, dts_out[:nsteps]
+
+
+def max_rate(p, U):
+    args, keep = _common(p)
+    S = _state(p, U)
+    return lib().oracle_max_rate(*args, *[_ptr(a) for a in S])
+
+
+def compute_dt(p, U, cfl):
+    return cfl / max_rate(p, U)
+
+
+def fill_ghosts(p, U):
+    """Returns the 5 padded arrays shaped (nz+4 or 1, ny+4, nx+4)."""
+    args, keep = _common(p)
+    S = _state(p, U)
+    nx, ny, nz = int(p["nx"]), int(p["ny"]), int(p["nz"])
+    shp = ((nz + 4) if nz > 1 else 1, ny + 4, nx + 4)
+    P = [np.zeros(shp) for _ in range(5)]
+    lib().oracle_fill_ghosts(*args, *[_ptr(a) for a in S], *[_ptr(a) for a in P])
+    return P
+
+
+def face(gamma, rhoL, unL, pL, rhoR, unR, pR, gh=0.0, theta_flag=1):
+    """-> dict(cL, cR, a, S, ustar, theta, pistar) for one face (pin P8)."""
+    out = np.zeros(7)
+    lib().oracle_face(gamma, rhoL, unL, pL, rhoR, unR, pR, gh, int(theta_flag), _ptr(out))
+    return dict(zip(["cL", "cR", "a", "S", "ustar", "theta", "pistar"], out.tolist()))
+
+
+def K():
+    return lib().oracle_K()
