@@ -1,0 +1,273 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s of the full ARK time step (compute_dt + step) on B200, with roofline and CPU baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one pass of the whole hot path over the synthetic workload: ghost fill (3 kernels), fused
+acoustic+transport+dissipative+update kernel with the CFL epilogue, the second reduction pass and the 16-byte
+device->host read of dt (ark_compute_dt) -- exactly the loop {dt = ark_compute_dt(cfl); ark_step(dt)}.
+
+Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs N independent
+replicas of the workload, one process per GPU (torchrun), no data-path collective; value = N * cells * K / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/sec per full time step (fp64)"
+UNIT = "cell-updates/s"
+CFL = 0.4
+
+WORKLOADS = {
+    # name: (builder name in inputs, n, bytes per cell update, oracle sample size)
+    "config5_512": ("config5_convection3d", 512, 80, 112),
+    "config4_256": ("config4_rb3d", 256, 80, 112),
+    "config3_1024x512": ("config3_rb2d", (1024, 512), 64, (512, 256)),
+    "config2_512": ("config2_gresho", 512, 64, 512),
+    "config1_128": ("config1_atmosphere", 128, 64, 128),
+}
+
+
+def build_workload(name, device=None, sample=False):
+    from paper_1903_09043_b200 import inputs
+    fn, n, bpc, ns = WORKLOADS[name]
+    size = ns if sample else n
+    f = getattr(inputs, fn)
+    if isinstance(size, tuple):
+        prm, U = f(size[0], size[1], device=device)
+    else:
+        prm, U = f(size, device=device)
+    return prm, U, bpc
+
+
+def measured_peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy_)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_timed(name, steps, warmup):
+    """The oracle as it stands, single thread, on a bounded sample of the workload (same recipe, smaller grid)."""
+    from oracle import ark_oracle as O
+    prm, U, bpc = build_workload(name, device=None, sample=True)
+    ncell = prm["nx"] * prm["ny"] * prm["nz"]
+    S = U
+    for _ in range(warmup):
+        S, _ = O.run(prm, S, 1, cfl=CFL)
+        S = [S[0], S[1], S[2], S[3] if prm["nz"] > 1 else None, S[4]]
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        S, _ = O.run(prm, S, 1, cfl=CFL)            # compute_dt + step, like the GPU loop
+        S = [S[0], S[1], S[2], S[3] if prm["nz"] > 1 else None, S[4]]
+    el = time.perf_counter() - t0
+    sample = "%s recipe at %dx%dx%d, %d steps of {compute_dt; step}, 1 thread" % (name, prm["nx"], prm["ny"], prm["nz"], steps)
+    return ncell * steps / el, el / steps * 1e3, sample
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    k = max(1, min(args.steps, 5))
+    val, ms, sample = oracle_timed(args.workload, k, 1)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
+            "warmup": 1, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "note": "oracle (oracle/ark_oracle.cpp) on host cores; each step is a bounded sample: " + sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    from paper_1903_09043_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    binding.load()
+    prm, U, bpc = build_workload(args.workload, device=dev)
+    U = [None if a is None else a.reshape(-1).contiguous() for a in U]
+    ncell = prm["nx"] * prm["ny"] * prm["nz"]
+    s = binding.Solver(prm, device=dev)
+    s.set_state(U)
+
+    W = max(args.warmup, 3)
+    K = args.steps
+    for _ in range(W):
+        s.step(s.compute_dt(CFL))
+    torch.cuda.synchronize()
+
+    # ---- timed region: K x {compute_dt; step}, device-timed on the solver's (= torch current) stream
+    s.step_kernel_timing(True)
+    l0 = s.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        s.step(s.compute_dt(CFL))
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    kern_ms, kern_n = s.step_kernel_time()
+    s.step_kernel_timing(False)
+    launches = s.launch_count() - l0
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * ncell * K / (ms_total * 1e-3)
+
+    # sanity: state still finite after the timed steps
+    dt_chk = s.compute_dt(CFL)
+    assert dt_chk > 0
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): set_state_host + compute_dt + step + get_state_host
+    e2e_steps = max(1, min(K, 3))
+    host_in = [None if a is None else a.cpu().pin_memory() for a in U]
+    host_out = [None if a is None else torch.empty_like(a) .pin_memory() for a in host_in]
+    nfield = sum(a is not None for a in host_in)
+    s.set_state_host(host_in)
+    s.step(s.compute_dt(CFL))
+    s.get_state_host(host_out)                      # warm-up of the e2e path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        s.set_state_host(host_in)
+        s.step(s.compute_dt(CFL))
+        s.get_state_host(host_out)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = world * ncell * e2e_steps / e2e_s
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        alg_bytes = bpc * ncell                       # per launch of the dominant (fused step) kernel
+        kern_avg_ms = kern_ms / max(kern_n, 1)
+        achieved = alg_bytes / (kern_avg_ms * 1e-3) / 1e9
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "grid": [prm["nx"], prm["ny"], prm["nz"]], "cfl": CFL,
+                           "step": "ark_compute_dt + ark_step (ghost fill x/y/z, fused step kernel, CFL pass 2, 16 B D2H)",
+                           "l2": "inputs larger than L2 (state %.2f GB)" % (bpc / 2 * ncell / 1e9) if bpc / 2 * ncell > 200e6
+                                 else "state fits in L2 (%.1f MB): latency-bound config, HBM roofline not meaningful" % (bpc / 2 * ncell / 1e6),
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "library": binding.version_string()},
+                "roofline": {"bound": "hbm", "kernel": "ark_k_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                             "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                             "algorithmic_bytes_per_cell": bpc, "kernel_ms": kern_avg_ms, "kernel_launches_timed": kern_n,
+                             "kernel_share_of_step": kern_ms / ms_total,
+                             "effective_whole_step_frac": bpc * value / world / 1e9 / peak},
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * 8,
+                        "d2h_bytes_per_step": nfield * ncell * 8 + 16, "steps": e2e_steps,
+                        "path": "ark_set_state_host + ark_compute_dt + ark_step + ark_get_state_host, pinned host buffers"},
+                "gpu_launches": launches, "clocks": clocks}
+        if world == 1 and not args.no_cpu_baseline:
+            val, ms, sample = oracle_timed(args.workload, 3, 1)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    s.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config5_512", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,109 @@
+/* ark.h -- C ABI of the B200-native (sm_100a) hot path of the ARK all-Mach solver (arXiv 1903.09043).
+ *
+ * One explicit finite-volume time step of the stratified compressible Euler / Navier-Stokes equations on a
+ * uniform 2D/3D Cartesian grid, fp64, single GPU:
+ *   ghost-cell fill -> acoustic step (u*, Pi*, L~, U~) -> transport step (upwind on u*) + viscous / heat
+ *   face fluxes -> conservative update, plus the CFL time-step max-reduction.
+ * "PAPER.md:<n>" cites /root/reference/PAPER.md; "A<n>" are the readings listed in DESIGN.md.
+ *
+ * Conventions
+ *   - All state arrays are DENSE interior-only fp64, nx*ny*nz elements, x fastest:
+ *       idx = i + nx*(j + ny*k).  rho, rho*u, rho*v, rho*w, E  with  E = rho*e + 1/2 rho |u|^2
+ *       (total energy density WITHOUT potential energy).
+ *   - nz == 1 selects 2D: the z axis and rho*w do not exist; rhow may be NULL.
+ *   - Pointers are DEVICE pointers unless the function name ends in _host.  The caller owns every
+ *     array it passes; the library copies into / out of its own padded SoA buffers and never
+ *     retains a caller pointer except the workspace.
+ *   - The workspace is caller-allocated device memory (PyTorch in this repo) of at least
+ *     ark_workspace_bytes() bytes, 256-byte aligned; it must outlive the handle.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call
+ *     enqueues on that stream; only the calls documented as synchronising wait for it.
+ *   - Every entry point returns an ARK_* code and never throws; ark_last_error() gives a text for
+ *     the last failure on the calling thread.
+ *   - Gravity is the constant vector g (Phi = -g.x, never stored: A12).  The acoustic impedance
+ *     constant is K = 1.1 (a = K max(rho_L c_L, rho_R c_R), A2), reported by
+ *     ark_version_string().
+ */
+#ifndef ARK_H
+#define ARK_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ark_solver ark_solver; /* opaque, owned by the library */
+
+enum { ARK_OK = 0, ARK_EINVAL = -1, ARK_ENOMEM = -2, ARK_ECUDA = -3, ARK_ENONFINITE = -4 };
+
+/* Boundary kinds (A9; PAPER.md:295 ghost zones, :378 reflecting + hydrostatic extrapolation,
+ * :457 fixed temperature).  Periodic must be set on both sides of an axis. */
+enum { ARK_BC_PERIODIC = 0, ARK_BC_REFLECTING = 1, ARK_BC_FIXED_T_WALL = 2 };
+
+typedef struct {
+    int type[3][2];     /* [axis x,y,z][lo,hi] */
+    double value[3][2]; /* wall temperature for ARK_BC_FIXED_T_WALL (T = p/rho, A8); ignored otherwise */
+} ark_bc;
+
+/* Bytes of device workspace ark_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */
+size_t ark_workspace_bytes(int nx, int ny, int nz);
+
+/* Create a solver.  nx,ny >= 4; nz >= 4 or nz == 1 (2D).  dx > 0 (uniform); gamma > 1
+ * (ideal gas); g[3] constant gravity; mu, kappa >= 0 constant dynamic
+ * viscosity and conductivity; low_mach_theta: 0 -> theta == 1, 1 -> eq. (13)
+ * (PAPER.md:218-222, 325).  d_workspace: device memory, see above.  Errors: ARK_EINVAL (bad argument,
+ * workspace too small or misaligned), ARK_ECUDA. */
+int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma, const double g[3],
+               double mu, double kappa, int low_mach_theta, const ark_bc* bc,
+               void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Copy a dense device state into the solver (asynchronous on the stream). */
+int ark_set_state(ark_solver*, const double* rho, const double* rhou, const double* rhov,
+                  const double* rhow, const double* E);
+/* Copy the current state out to dense device arrays (asynchronous on the stream). */
+int ark_get_state(ark_solver*, double* rho, double* rhou, double* rhov, double* rhow, double* E);
+
+/* Same with HOST arrays (pageable or pinned).  The copies run on the stream through a staging
+ * area inside the workspace; both calls return after the stream has been synchronised. */
+int ark_set_state_host(ark_solver*, const double* rho, const double* rhou, const double* rhov,
+                       const double* rhow, const double* E);
+int ark_get_state_host(ark_solver*, double* rho, double* rhou, double* rhov, double* rhow, double* E);
+
+/* CFL time step ("time step kernel"; formula = A4):
+ *   dt = cfl / max_c [ sum_d (|u_d| + c)/dx + 2 ndim max(4 mu/3, (gamma-1) kappa) / (rho dx^2) ].
+ * Deterministic two-pass max reduction (NaN-propagating).  Synchronises the stream (8-byte D2H).
+ * Returns ARK_ENONFINITE if the maximum rate is not finite and positive. */
+int ark_compute_dt(ark_solver*, double cfl, double* dt_out);
+
+/* Advance the state by one full step of size dt (ghost fill, acoustic + transport + dissipative
+ * fluxes, conservative update).  Asynchronous on the stream. */
+int ark_step(ark_solver*, double dt);
+
+/* Convenience: nsteps x { dt = cfl / max rate ; step(dt) } with the time step kept on the device
+ * (no host round trip per step).  If dts_out (HOST, nsteps doubles) is not NULL the step sizes are
+ * copied there; the call then synchronises.  Returns ARK_ENONFINITE if a rate was not finite. */
+int ark_run(ark_solver*, int nsteps, double cfl, double* dts_out);
+
+/* Ghost fill only, then copy the PADDED current state ((nx+4)*(ny+4)*(nz+4 or 1) per field, x fastest)
+ * to device arrays: test hook for the boundary kernel.  Asynchronous. */
+int ark_debug_get_padded(ark_solver*, double* rho, double* rhou, double* rhov, double* rhow, double* E);
+
+/* Measurement hook: when enabled, every launch of the fused step kernel is bracketed by CUDA events on the
+ * solver's stream (up to 4096 launches are kept; older ones are dropped).  ark_step_kernel_time() synchronises
+ * the stream and returns the summed device time in milliseconds and the number of launches measured since
+ * the last ark_step_kernel_timing(.., 1) call. */
+int ark_step_kernel_timing(ark_solver*, int enable);
+int ark_step_kernel_time(ark_solver*, double* total_ms, int* launches);
+
+/* Number of kernels this library has launched on behalf of the handle since creation. */
+long long ark_launch_count(const ark_solver*);
+
+void ark_destroy(ark_solver*);
+const char* ark_last_error(void);
+const char* ark_version_string(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARK_H */

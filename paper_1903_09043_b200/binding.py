@@ -1,0 +1,205 @@
+"""Thin Python binding of the C-ABI library (include/ark.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libark_b200.so; PyTorch is used for device
+memory (the workspace, the dense state tensors) and the stream.  There is no CPU fallback: if the
+library is missing or cannot be loaded this module raises.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libark_b200.so")
+
+ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
+BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL = 0, 1, 2
+
+EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
+           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_debug_get_padded",
+           "ark_step_kernel_timing", "ark_step_kernel_time", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
+
+
+class ark_bc(C.Structure):
+    _fields_ = [("type", (C.c_int * 2) * 3), ("value", (C.c_double * 2) * 3)]
+
+
+class ArkError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("ark error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def load():
+    """dlopen libark_b200.so (built in-tree by `python -m paper_1903_09043_b200.build`) and declare prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("%s not found: build it with `python -m paper_1903_09043_b200.build` "
+                          "(no CPU fallback exists)" % LIB_PATH)
+    lib = C.CDLL(LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.c_int
+    lib.ark_workspace_bytes.argtypes = [ip, ip, ip]
+    lib.ark_workspace_bytes.restype = C.c_size_t
+    lib.ark_create.argtypes = [C.POINTER(vp), ip, ip, ip, C.c_double, C.c_double, C.POINTER(C.c_double),
+                               C.c_double, C.c_double, ip, C.POINTER(ark_bc), vp, C.c_size_t, vp]
+    lib.ark_create.restype = ip
+    for name in ("ark_set_state", "ark_get_state", "ark_set_state_host", "ark_get_state_host", "ark_debug_get_padded"):
+        getattr(lib, name).argtypes = [vp] + [dp] * 5
+        getattr(lib, name).restype = ip
+    lib.ark_compute_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
+    lib.ark_compute_dt.restype = ip
+    lib.ark_step.argtypes = [vp, C.c_double]
+    lib.ark_step.restype = ip
+    lib.ark_run.argtypes = [vp, ip, C.c_double, C.POINTER(C.c_double)]
+    lib.ark_run.restype = ip
+    lib.ark_step_kernel_timing.argtypes = [vp, ip]
+    lib.ark_step_kernel_timing.restype = ip
+    lib.ark_step_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    lib.ark_step_kernel_time.restype = ip
+    lib.ark_launch_count.argtypes = [vp]
+    lib.ark_launch_count.restype = C.c_longlong
+    lib.ark_destroy.argtypes = [vp]
+    lib.ark_destroy.restype = None
+    lib.ark_last_error.restype = C.c_char_p
+    lib.ark_version_string.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def version_string():
+    return load().ark_version_string().decode()
+
+
+def workspace_bytes(nx, ny, nz):
+    return int(load().ark_workspace_bytes(nx, ny, nz))
+
+
+def _check(rc):
+    if rc != ARK_OK:
+        raise ArkError(rc, load().ark_last_error().decode())
+
+
+class Solver:
+    """ark_create / ark_set_state / ark_get_state / ark_compute_dt / ark_step / ark_run / ark_destroy.
+
+    params: dict(nx, ny, nz, dx, gamma, g, mu, kappa, theta, bc_type[3][2], bc_value[3][2]) as produced by
+    `paper_1903_09043_b200.inputs`.  State tensors are dense float64 CUDA tensors of nx*ny*nz elements
+    (x fastest); rhow is None in 2D.
+    """
+
+    def __init__(self, params, device="cuda:0", stream=None):
+        lib = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1903_09043_b200 needs a CUDA device (no CPU fallback)")
+        self.p = dict(params)
+        self.device = torch.device(device)
+        self.nx, self.ny, self.nz = int(params["nx"]), int(params["ny"]), int(params["nz"])
+        self.n = self.nx * self.ny * self.nz
+        self.ndim = 3 if self.nz > 1 else 2
+        nbytes = lib.ark_workspace_bytes(self.nx, self.ny, self.nz)
+        if nbytes == 0:
+            raise ArkError(ARK_EINVAL, "invalid grid size")
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        base = self.workspace.data_ptr()
+        self._ws_ptr = (base + 255) // 256 * 256
+        bc = ark_bc()
+        for d in range(3):
+            for s in range(2):
+                bc.type[d][s] = int(params["bc_type"][d][s])
+                bc.value[d][s] = float(params["bc_value"][d][s])
+        g = (C.c_double * 3)(*[float(x) for x in params["g"]])
+        h = C.c_void_p()
+        _check(lib.ark_create(C.byref(h), self.nx, self.ny, self.nz, float(params["dx"]), float(params["gamma"]), g,
+                              float(params["mu"]), float(params["kappa"]), int(params["theta"]), C.byref(bc),
+                              C.c_void_p(self._ws_ptr), C.c_size_t(nbytes), C.c_void_p(self.stream.cuda_stream)))
+        self._h = h
+        self._lib = lib
+
+    # ------------------------------------------------------------------ state
+    def _ptrs(self, U, host=False):
+        out = []
+        for f, a in enumerate(U):
+            if a is None:
+                if not (f == 3 and self.ndim == 2):
+                    raise ValueError("state field %d is None" % f)
+                out.append(None)
+                continue
+            if a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != self.n:
+                raise ValueError("state field %d must be a contiguous float64 tensor of %d elements" % (f, self.n))
+            if host != (a.device.type == "cpu"):
+                raise ValueError("state field %d is on %s" % (f, a.device))
+            out.append(C.c_void_p(a.data_ptr()))
+        return out
+
+    def set_state(self, U):
+        _check(self._lib.ark_set_state(self._h, *self._ptrs(U)))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = [torch.empty(self.n, dtype=torch.float64, device=self.device) if not (f == 3 and self.ndim == 2) else None
+                   for f in range(5)]
+        _check(self._lib.ark_get_state(self._h, *self._ptrs(out)))
+        return out
+
+    def set_state_host(self, U):
+        _check(self._lib.ark_set_state_host(self._h, *self._ptrs(U, host=True)))
+
+    def get_state_host(self, out):
+        _check(self._lib.ark_get_state_host(self._h, *self._ptrs(out, host=True)))
+        return out
+
+    def get_padded(self):
+        """ghost-filled padded state: list of tensors shaped (nz+4 or 1, ny+4, nx+4) (test hook)."""
+        shp = ((self.nz + 4) if self.ndim == 3 else 1, self.ny + 4, self.nx + 4)
+        out = [torch.empty(shp, dtype=torch.float64, device=self.device) if not (f == 3 and self.ndim == 2) else None
+               for f in range(5)]
+        ptrs = [None if a is None else C.c_void_p(a.data_ptr()) for a in out]
+        _check(self._lib.ark_debug_get_padded(self._h, *ptrs))
+        return out
+
+    # ------------------------------------------------------------------ time stepping
+    def compute_dt(self, cfl):
+        dt = C.c_double()
+        _check(self._lib.ark_compute_dt(self._h, float(cfl), C.byref(dt)))
+        return dt.value
+
+    def step(self, dt):
+        _check(self._lib.ark_step(self._h, float(dt)))
+
+    def run(self, nsteps, cfl, want_dts=False):
+        if want_dts:
+            buf = (C.c_double * max(nsteps, 1))()
+            _check(self._lib.ark_run(self._h, int(nsteps), float(cfl), buf))
+            return list(buf)[:nsteps]
+        _check(self._lib.ark_run(self._h, int(nsteps), float(cfl), None))
+        return None
+
+    def step_kernel_timing(self, enable=True):
+        _check(self._lib.ark_step_kernel_timing(self._h, int(bool(enable))))
+
+    def step_kernel_time(self):
+        """-> (total milliseconds, launches) of the fused step kernel since timing was enabled."""
+        ms, n = C.c_double(), C.c_int()
+        _check(self._lib.ark_step_kernel_time(self._h, C.byref(ms), C.byref(n)))
+        return ms.value, n.value
+
+    def launch_count(self):
+        return int(self._lib.ark_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.ark_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

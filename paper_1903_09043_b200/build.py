@@ -1,0 +1,35 @@
+"""Build the CUDA C-ABI library in-tree:  python -m paper_1903_09043_b200.build
+
+nvcc cross-compiles for sm_100a without a GPU.  The .so is git-ignored but travels to the GPU box.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libark_b200.so")
+SOURCES = ["ark.cu"]
+HEADERS = ["ark_device.cuh", "ark_step.cuh", os.path.join("..", "..", "include", "ark.h")]
+# tile of the fused step kernel: (TX, TY) outputs per block and plane, region (TX+4) x (TY+4) threads
+TILES = {"ARK_TX3": 32, "ARK_TY3": 8, "ARK_TX2": 32, "ARK_TY2": 8}
+
+
+def nvcc_cmd(out, extra=()):
+    defs = ["-D%s=%d" % kv for kv in TILES.items()]
+    return (["nvcc", "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+             "-Xcompiler", "-fPIC", "-shared", "-o", out] + defs + list(extra)
+            + [os.path.join(CSRC, s) for s in SOURCES])
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+        return LIB
+    cmd = nvcc_cmd(LIB, ["-Xptxas", "-v"] if verbose else [])
+    subprocess.run(cmd, check=True)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,414 @@
+// ark.cu -- C-ABI implementation (include/ark.h) on top of the sm_100a kernels in ark_device.cuh / ark_step.cuh.
+// No torch types, no CPU fallback: every step of the hot path runs in the kernels of this library.
+#include "../../include/ark.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ark_step.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, const char* a = "", long long b = 0) {
+    snprintf(g_err, sizeof g_err, fmt, a, b);
+    return code;
+}
+#define ARK_CUDA(call)                                                             \
+    do {                                                                           \
+        cudaError_t e_ = (call);                                                   \
+        if (e_ != cudaSuccess) return fail(ARK_ECUDA, "CUDA error: %s (%lld)", cudaGetErrorString(e_), (long long)__LINE__); \
+    } while (0)
+
+// tile of the fused step kernel
+constexpr int TX3 = ARK_TX3, TY3 = ARK_TY3;   // 3D
+constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
+
+constexpr int CFL_BLOCK = 256;
+#define ARK_MAX_TIMED 4096
+constexpr int MAX_SCRATCH = 1 << 16;          // per-block rate slots
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+    int px, py, pz, offz, nf;
+    long long fstride;       // doubles
+    size_t state_bytes;      // one padded state (nf fields)
+    size_t scratch_off, result_off, dtlog_off, stage_off, total;
+};
+
+bool valid_sizes(int nx, int ny, int nz) {
+    return nx >= 4 && ny >= 4 && (nz == 1 || nz >= 4) && nx <= (1 << 14) && ny <= (1 << 14) && nz <= (1 << 14);
+}
+
+constexpr int DTLOG_MAX = 1 << 16;
+
+Layout make_layout(int nx, int ny, int nz) {
+    Layout L;
+    const bool d3 = nz > 1;
+    L.nf = d3 ? 5 : 4;
+    L.offz = d3 ? ARK_NG : 0;
+    L.px = (int)round_up((size_t)nx + 2 * ARK_NG, 16);
+    L.py = ny + 2 * ARK_NG;
+    L.pz = d3 ? nz + 2 * ARK_NG : 1;
+    L.fstride = (long long)round_up((size_t)L.px * L.py * L.pz, 32);
+    L.state_bytes = (size_t)L.nf * L.fstride * sizeof(double);
+    size_t off = 2 * L.state_bytes;
+    L.scratch_off = off; off += round_up((size_t)MAX_SCRATCH * sizeof(double), 256);
+    L.result_off = off;  off += 256;
+    L.dtlog_off = off;   off += round_up((size_t)DTLOG_MAX * sizeof(double), 256);
+    L.stage_off = off;   off += round_up((size_t)nx * ny * nz * sizeof(double), 256);   // one dense field (host copies)
+    L.total = off;
+    return L;
+}
+
+}  // namespace
+
+struct ark_solver {
+    ArkParams P;
+    Layout L;
+    char* ws;
+    double* U[2];           // padded states; U[cur] holds the current one
+    int cur;
+    double* scratch;        // per-block rates
+    double* result;         // [0] max rate, [1] dt
+    double* dtlog;
+    double* stage;
+    cudaStream_t stream;
+    int rate_slots;         // >0: scratch[0..rate_slots) holds the per-block rates of the CURRENT state
+    dim3 step_grid;
+    int zchunk;
+    long long launches;
+    double* h_pinned;       // 2 doubles, pinned, for the 16-byte D2H of compute_dt
+    // optional event bracketing of the step kernel (measurement hook)
+    bool timing;
+    int n_timed;
+    cudaEvent_t ev0[ARK_MAX_TIMED], ev1[ARK_MAX_TIMED];
+    bool ev_created;
+};
+
+namespace {
+
+int grid_for(long long n, int block, int cap = 148 * 8) {
+    long long b = (n + block - 1) / block;
+    if (b < 1) b = 1;
+    return (int)(b < cap ? b : cap);
+}
+
+template <int NDIM, bool VISC, int TX, int TY>
+int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
+    using C = ArkStepCfg<TX, TY>;
+    static bool attr_set = false;
+    auto kern = ark_k_step<NDIM, VISC, TX, TY>;
+    if (!attr_set) {
+        ARK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+        attr_set = true;
+    }
+    const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
+    if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
+    kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
+                                                            s->scratch, s->zchunk);
+    if (timed) { ARK_CUDA(cudaEventRecord(s->ev1[s->n_timed], s->stream)); s->n_timed++; }
+    ARK_CUDA(cudaGetLastError());
+    s->launches++;
+    return ARK_OK;
+}
+
+int launch_bc(ark_solver* s, double* U) {
+    const ArkParams& P = s->P;
+    {
+        const long long n = 2LL * P.ny * P.nz;
+        ark_k_bc<0><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
+    }
+    {
+        const long long n = 2LL * (P.nx + 2 * ARK_NG) * P.nz;
+        ark_k_bc<1><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
+    }
+    s->launches += 2;
+    if (P.ndim == 3) {
+        const long long n = 2LL * (P.nx + 2 * ARK_NG) * (P.ny + 2 * ARK_NG);
+        ark_k_bc<2><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+int do_step(ark_solver* s, double dt, const double* dt_dev) {
+    int rc = launch_bc(s, s->U[s->cur]);
+    if (rc != ARK_OK) return rc;
+    const bool visc = s->P.mu > 0.0 || s->P.kappa > 0.0;
+    if (s->P.ndim == 3) rc = visc ? launch_step_t<3, true, TX3, TY3>(s, dt, dt_dev) : launch_step_t<3, false, TX3, TY3>(s, dt, dt_dev);
+    else                rc = visc ? launch_step_t<2, true, TX2, TY2>(s, dt, dt_dev) : launch_step_t<2, false, TX2, TY2>(s, dt, dt_dev);
+    if (rc != ARK_OK) return rc;
+    s->cur = 1 - s->cur;
+    s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
+    return ARK_OK;
+}
+
+// max rate of the current state -> result[0], dt -> result[1] (device).  Uses the step kernel's epilogue
+// values when they describe the current state, otherwise runs the standalone pass 1.
+int reduce_rate(ark_solver* s, double cfl, double* dt_log, int step_index) {
+    int nvals = s->rate_slots;
+    if (nvals <= 0) {
+        const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+        nvals = grid_for(n, CFL_BLOCK, 148 * 8);
+        ark_k_cfl_pass1<<<nvals, CFL_BLOCK, 0, s->stream>>>(s->P, s->U[s->cur], s->scratch);
+        s->launches++;
+        s->rate_slots = nvals;
+    }
+    ark_k_cfl_pass2<<<1, 1024, 0, s->stream>>>(s->scratch, nvals, cfl, s->result, dt_log, step_index);
+    s->launches++;
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ark_last_error(void) { return g_err; }
+
+const char* ark_version_string(void) {
+    static char buf[256];
+    snprintf(buf, sizeof buf, "ark-b200 0.1 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d tile2d=%dx%d)", ARK_K_IMPEDANCE, ARK_NG,
+             TX3, TY3, TX2, TY2);
+    return buf;
+}
+
+size_t ark_workspace_bytes(int nx, int ny, int nz) {
+    if (!valid_sizes(nx, ny, nz)) return 0;
+    return make_layout(nx, ny, nz).total;
+}
+
+int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma, const double g[3], double mu,
+               double kappa, int low_mach_theta, const ark_bc* bc, void* d_workspace, size_t workspace_bytes,
+               void* cuda_stream) {
+    if (!out) return fail(ARK_EINVAL, "ark_create: out is NULL%s");
+    *out = nullptr;
+    if (!valid_sizes(nx, ny, nz)) return fail(ARK_EINVAL, "ark_create: need nx,ny >= 4 and nz == 1 or nz >= 4%s");
+    if (!(dx > 0.0) || !(gamma > 1.0) || !(mu >= 0.0) || !(kappa >= 0.0) || !g || !bc)
+        return fail(ARK_EINVAL, "ark_create: need dx > 0, gamma > 1, mu,kappa >= 0, g and bc non-NULL%s");
+    if (low_mach_theta != 0 && low_mach_theta != 1) return fail(ARK_EINVAL, "ark_create: low_mach_theta must be 0 or 1%s");
+    const int ndim = nz > 1 ? 3 : 2;
+    for (int d = 0; d < ndim; ++d) {
+        for (int sd = 0; sd < 2; ++sd) {
+            const int t = bc->type[d][sd];
+            if (t != ARK_BC_PERIODIC && t != ARK_BC_REFLECTING && t != ARK_BC_FIXED_T_WALL)
+                return fail(ARK_EINVAL, "ark_create: unknown boundary kind%s");
+            if (t == ARK_BC_FIXED_T_WALL && !(bc->value[d][sd] > 0.0))
+                return fail(ARK_EINVAL, "ark_create: fixed-T wall needs a positive temperature%s");
+        }
+        if ((bc->type[d][0] == ARK_BC_PERIODIC) != (bc->type[d][1] == ARK_BC_PERIODIC))
+            return fail(ARK_EINVAL, "ark_create: periodic must be set on both sides of an axis%s");
+    }
+    const Layout L = make_layout(nx, ny, nz);
+    if (!d_workspace || workspace_bytes < L.total || ((size_t)d_workspace & 255))
+        return fail(ARK_EINVAL, "ark_create: workspace NULL, misaligned (256 B) or smaller than ark_workspace_bytes()%s");
+
+    ark_solver* s = new (std::nothrow) ark_solver;
+    if (!s) return fail(ARK_ENOMEM, "ark_create: out of host memory%s");
+    memset(s, 0, sizeof *s);
+    ArkParams& P = s->P;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.ndim = ndim; P.nf = L.nf;
+    P.px = L.px; P.py = L.py; P.pz = L.pz; P.offz = L.offz; P.fstride = L.fstride;
+    P.h = dx; P.gamma = gamma; P.gm1 = gamma - 1.0; P.mu = mu; P.kappa = kappa; P.theta = low_mach_theta;
+    for (int d = 0; d < 3; ++d) {
+        P.g[d] = d < ndim ? g[d] : 0.0;
+        for (int sd = 0; sd < 2; ++sd) { P.bc[d][sd] = bc->type[d][sd]; P.bcv[d][sd] = bc->value[d][sd]; }
+    }
+    s->L = L;
+    s->ws = (char*)d_workspace;
+    s->U[0] = (double*)s->ws;
+    s->U[1] = (double*)(s->ws + L.state_bytes);
+    s->cur = 0;
+    s->scratch = (double*)(s->ws + L.scratch_off);
+    s->result = (double*)(s->ws + L.result_off);
+    s->dtlog = (double*)(s->ws + L.dtlog_off);
+    s->stage = (double*)(s->ws + L.stage_off);
+    s->stream = (cudaStream_t)cuda_stream;
+    s->rate_slots = 0;
+    s->launches = 0;
+
+    // launch geometry of the fused step kernel
+    if (ndim == 3) {
+        const int gx = (nx + TX3 - 1) / TX3, gy = (ny + TY3 - 1) / TY3;
+        // z chunks: enough blocks for >= ~4 waves of 148 SMs, chunk length >= 16 planes (prologue = 2 planes)
+        int nchunk = 1;
+        while (nchunk < nz / 16 && (long long)gx * gy * nchunk < 148LL * 4) nchunk *= 2;
+        int zc = (nz + nchunk - 1) / nchunk;
+        nchunk = (nz + zc - 1) / zc;
+        s->zchunk = zc;
+        s->step_grid = dim3(gx, gy, nchunk);
+    } else {
+        s->zchunk = 1;
+        s->step_grid = dim3((nx + TX2 - 1) / TX2, (ny + TY2 - 1) / TY2, 1);
+    }
+    if ((long long)s->step_grid.x * s->step_grid.y * s->step_grid.z > MAX_SCRATCH) {
+        delete s;
+        return fail(ARK_EINVAL, "ark_create: grid too large for the rate scratch%s");
+    }
+    cudaError_t e = cudaMallocHost((void**)&s->h_pinned, 2 * sizeof(double));
+    if (e != cudaSuccess) { delete s; return fail(ARK_ECUDA, "CUDA error: %s", cudaGetErrorString(e)); }
+    // ghost cells and padding start finite (they are read by clamped / halo threads before the first fill)
+    e = cudaMemsetAsync(s->ws, 0, L.total, s->stream);
+    if (e != cudaSuccess) { cudaFreeHost(s->h_pinned); delete s; return fail(ARK_ECUDA, "CUDA error: %s", cudaGetErrorString(e)); }
+    *out = s;
+    return ARK_OK;
+}
+
+int ark_step_kernel_timing(ark_solver* s, int enable) {
+    if (!s) return fail(ARK_EINVAL, "ark_step_kernel_timing: NULL handle%s");
+    if (enable && !s->ev_created) {
+        for (int i = 0; i < ARK_MAX_TIMED; ++i) {
+            ARK_CUDA(cudaEventCreate(&s->ev0[i]));
+            ARK_CUDA(cudaEventCreate(&s->ev1[i]));
+        }
+        s->ev_created = true;
+    }
+    s->timing = enable != 0;
+    s->n_timed = 0;
+    return ARK_OK;
+}
+
+int ark_step_kernel_time(ark_solver* s, double* total_ms, int* launches) {
+    if (!s || !total_ms || !launches) return fail(ARK_EINVAL, "ark_step_kernel_time: NULL argument%s");
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    double sum = 0.0;
+    for (int i = 0; i < s->n_timed; ++i) {
+        float ms = 0.f;
+        ARK_CUDA(cudaEventElapsedTime(&ms, s->ev0[i], s->ev1[i]));
+        sum += ms;
+    }
+    *total_ms = sum;
+    *launches = s->n_timed;
+    return ARK_OK;
+}
+
+void ark_destroy(ark_solver* s) {
+    if (!s) return;
+    if (s->ev_created)
+        for (int i = 0; i < ARK_MAX_TIMED; ++i) { cudaEventDestroy(s->ev0[i]); cudaEventDestroy(s->ev1[i]); }
+    if (s->h_pinned) cudaFreeHost(s->h_pinned);
+    delete s;
+}
+
+long long ark_launch_count(const ark_solver* s) { return s ? s->launches : 0; }
+
+int ark_set_state(ark_solver* s, const double* rho, const double* rhou, const double* rhov, const double* rhow,
+                  const double* E) {
+    if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_set_state: NULL argument%s");
+    const double* src[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
+    const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+    for (int f = 0; f < s->P.nf; ++f) {
+        ark_k_pack<<<grid_for(n, 256), 256, 0, s->stream>>>(s->P, s->U[s->cur], (s->P.ndim == 3 || f < 3) ? src[f] : E, f);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    s->rate_slots = 0;
+    return ARK_OK;
+}
+
+int ark_get_state(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
+    if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_get_state: NULL argument%s");
+    double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
+    const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+    for (int f = 0; f < s->P.nf; ++f) {
+        ark_k_unpack<<<grid_for(n, 256), 256, 0, s->stream>>>(s->P, s->U[s->cur], (s->P.ndim == 3 || f < 3) ? dst[f] : E, f);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+int ark_set_state_host(ark_solver* s, const double* rho, const double* rhou, const double* rhov, const double* rhow,
+                       const double* E) {
+    if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_set_state_host: NULL argument%s");
+    const double* src[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
+    const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+    for (int f = 0; f < s->P.nf; ++f) {
+        const double* h = (s->P.ndim == 3 || f < 3) ? src[f] : E;
+        ARK_CUDA(cudaMemcpyAsync(s->stage, h, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+        ark_k_pack<<<grid_for(n, 256), 256, 0, s->stream>>>(s->P, s->U[s->cur], s->stage, f);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    s->rate_slots = 0;
+    return ARK_OK;
+}
+
+int ark_get_state_host(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
+    if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_get_state_host: NULL argument%s");
+    double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
+    const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+    for (int f = 0; f < s->P.nf; ++f) {
+        double* h = (s->P.ndim == 3 || f < 3) ? dst[f] : E;
+        ark_k_unpack<<<grid_for(n, 256), 256, 0, s->stream>>>(s->P, s->U[s->cur], s->stage, f);
+        s->launches++;
+        ARK_CUDA(cudaMemcpyAsync(h, s->stage, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    }
+    ARK_CUDA(cudaGetLastError());
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    return ARK_OK;
+}
+
+int ark_compute_dt(ark_solver* s, double cfl, double* dt_out) {
+    if (!s || !dt_out || !(cfl > 0.0)) return fail(ARK_EINVAL, "ark_compute_dt: bad argument%s");
+    int rc = reduce_rate(s, cfl, nullptr, 0);
+    if (rc != ARK_OK) return rc;
+    ARK_CUDA(cudaMemcpyAsync(s->h_pinned, s->result, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    const double rate = s->h_pinned[0];
+    if (!(rate > 0.0) || std::isinf(rate) || std::isnan(rate)) {
+        *dt_out = std::nan("");
+        return fail(ARK_ENONFINITE, "ark_compute_dt: maximum CFL rate is not finite and positive%s");
+    }
+    *dt_out = cfl / rate;
+    return ARK_OK;
+}
+
+int ark_step(ark_solver* s, double dt) {
+    if (!s || !(dt > 0.0) || std::isinf(dt)) return fail(ARK_EINVAL, "ark_step: dt must be finite and positive%s");
+    return do_step(s, dt, nullptr);
+}
+
+int ark_run(ark_solver* s, int nsteps, double cfl, double* dts_out) {
+    if (!s || nsteps < 0 || !(cfl > 0.0)) return fail(ARK_EINVAL, "ark_run: bad argument%s");
+    if (dts_out && nsteps > DTLOG_MAX) return fail(ARK_EINVAL, "ark_run: at most %s%lld steps when dts_out is given", "", (long long)DTLOG_MAX);
+    for (int i = 0; i < nsteps; ++i) {
+        int rc = reduce_rate(s, cfl, dts_out ? s->dtlog : nullptr, i);
+        if (rc != ARK_OK) return rc;
+        rc = do_step(s, 0.0, s->result);
+        if (rc != ARK_OK) return rc;
+    }
+    if (dts_out && nsteps > 0) {
+        ARK_CUDA(cudaMemcpyAsync(dts_out, s->dtlog, (size_t)nsteps * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        ARK_CUDA(cudaStreamSynchronize(s->stream));
+        for (int i = 0; i < nsteps; ++i)
+            if (!(dts_out[i] > 0.0) || std::isinf(dts_out[i]))
+                return fail(ARK_ENONFINITE, "ark_run: non-finite CFL rate at step %s%lld", "", (long long)i);
+    }
+    return ARK_OK;
+}
+
+int ark_debug_get_padded(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
+    if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_debug_get_padded: NULL argument%s");
+    int rc = launch_bc(s, s->U[s->cur]);
+    if (rc != ARK_OK) return rc;
+    double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
+    const long long n = (long long)(s->P.nx + 2 * ARK_NG) * s->P.py * s->P.pz;
+    for (int f = 0; f < s->P.nf; ++f) {
+        ark_k_unpack_padded<<<grid_for(n, 256), 256, 0, s->stream>>>(s->P, s->U[s->cur], (s->P.ndim == 3 || f < 3) ? dst[f] : E, f);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,261 @@
+// ark_device.cuh -- device-side data layout and kernels of the ARK hot path (sm_100a).
+//
+// Scheme: PAPER.md (arXiv 1903.09043) sections 2.1-2.2 with readings A1..A20 of DESIGN.md.
+// This file shares nothing with oracle/: every formula is restated here from the paper.
+//
+// HBM layout: SoA fp64, one padded array per conserved field (rho, rho*u, rho*v, [rho*w], E),
+// 2 ghost layers per side (A9), x fastest, row pitch px (multiple of 16 doubles = 128 B), so the
+// halo'd tile of a block starts on a 128-byte boundary whenever the tile origin is a multiple of 16.
+#pragma once
+
+#ifndef ARK_HOST_EMU
+#include <cuda_runtime.h>
+#define ARK_DEV __device__ __forceinline__
+#define ARK_GLOBAL __global__
+#define ARK_SHARED __shared__
+#define ARK_DYN_SMEM(name) extern __shared__ double name[]
+#else
+// host emulation shim (debugging aid outside the product build): supplies threadIdx & co, __syncthreads, rsqrt
+#include "ark_emu.h"
+#endif
+
+#define ARK_K_IMPEDANCE 1.1  // a = K max(rho_L c_L, rho_R c_R), reading A2
+#define ARK_NG 2             // ghost layers (A9)
+
+enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2 };
+
+struct ArkParams {
+    int nx, ny, nz, ndim, nf;   // interior sizes; nf = 4 (2D) or 5 (3D) stored fields
+    int px, py, pz;             // padded extents (px is the row pitch)
+    int offz;                   // 2 in 3D, 0 in 2D
+    long long fstride;          // doubles between consecutive fields
+    double h, gamma, gm1, g[3], mu, kappa;
+    int theta;                  // 0: theta == 1 ; 1: eq. (13)
+    int bc[3][2];
+    double bcv[3][2];
+};
+
+// padded linear index of interior-based cell (i,j,k); ghosts are -2,-1 and n,n+1
+ARK_DEV long long ark_idx(const ArkParams& P, int i, int j, int k) {
+    return (long long)(i + ARK_NG) + (long long)P.px * ((long long)(j + ARK_NG) + (long long)P.py * (long long)(k + P.offz));
+}
+
+// NaN-propagating max (fmax would drop NaNs): SURVEY 8(a) row 8
+ARK_DEV double ark_nanmax(double a, double b) { return (a != a) ? a : ((b != b) ? b : (a > b ? a : b)); }
+
+// ------------------------------------------------------------------------------------------------
+// Primitive variables of one cell (PAPER.md:315-319 ideal gas, c^2 = gamma p / rho; :370 p = rho T).
+// rc = rho*c and irc = 1/(rho*c) come from ONE rsqrt: rho*c = sqrt(gamma p rho).
+// ------------------------------------------------------------------------------------------------
+struct ArkPrim { double rho, u, v, w, p, rc, irc, T; };
+
+ARK_DEV ArkPrim ark_prim(const ArkParams& P, double rho, double mx, double my, double mz, double E) {
+    ArkPrim q;
+    const double rinv = 1.0 / rho;
+    q.rho = rho;
+    q.u = mx * rinv;
+    q.v = my * rinv;
+    q.w = mz * rinv;
+    const double ke = 0.5 * (mx * q.u + my * q.v + mz * q.w);
+    q.p = P.gm1 * (E - ke);
+    const double gpr = P.gamma * q.p * rho;        // (rho c)^2
+    q.irc = rsqrt(gpr);
+    q.rc = gpr * q.irc;
+    q.T = q.p * rinv;
+    return q;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Acoustic face between L and R along one axis (PAPER.md:152 for a, S, u*, Pi*; PAPER.md:218-222
+// for theta, eq. 13).  un = face-normal velocity, gh = g_d * h (Phi_R - Phi_L = -g_d h, A12).
+// Divisions by a and by max(c_L,c_R) are replaced by min() of the per-cell reciprocals:
+//   1/(2a) = min(irc_L, irc_R)/(2K),  1/max(c_L,c_R) = min(rho_L irc_L, rho_R irc_R).
+// ------------------------------------------------------------------------------------------------
+struct ArkFace { double us, pi, S; };
+
+ARK_DEV ArkFace ark_face(int theta_on, double gh,
+                         double rhoL, double unL, double pL, double rcL, double ircL,
+                         double rhoR, double unR, double pR, double rcR, double ircR) {
+    ArkFace f;
+    const double a = ARK_K_IMPEDANCE * fmax(rcL, rcR);
+    const double i2a = (0.5 / ARK_K_IMPEDANCE) * fmin(ircL, ircR);
+    f.S = (0.5 * gh) * (rhoL + rhoR);
+    f.us = 0.5 * (unL + unR) - ((pR - pL) - f.S) * i2a;
+    double ath = a;
+    if (theta_on) {
+        const double icm = fmin(rhoL * ircL, rhoR * ircR);
+        ath = a * fmin(fabs(f.us) * icm, 1.0);
+    }
+    f.pi = 0.5 * (pL + pR) - 0.5 * ath * (unR - unL);
+    return f;
+}
+
+// ------------------------------------------------------------------------------------------------
+// dense <-> padded copies
+// ------------------------------------------------------------------------------------------------
+ARK_GLOBAL void ark_k_pack(ArkParams P, double* __restrict__ U, const double* __restrict__ src, int field) {
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(s % P.nx);
+        const long long r = s / P.nx;
+        const int j = (int)(r % P.ny), k = (int)(r / P.ny);
+        U[field * P.fstride + ark_idx(P, i, j, k)] = src[s];
+    }
+}
+
+ARK_GLOBAL void ark_k_unpack(ArkParams P, const double* __restrict__ U, double* __restrict__ dst, int field) {
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(s % P.nx);
+        const long long r = s / P.nx;
+        const int j = (int)(r % P.ny), k = (int)(r / P.ny);
+        dst[s] = U[field * P.fstride + ark_idx(P, i, j, k)];
+    }
+}
+
+// padded (pitch px) -> padded dense (pitch nx+4): debug / test hook for the ghost fill
+ARK_GLOBAL void ark_k_unpack_padded(ArkParams P, const double* __restrict__ U, double* __restrict__ dst, int field) {
+    const int mx = P.nx + 2 * ARK_NG;
+    const long long n = (long long)mx * P.py * P.pz;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(s % mx);
+        const long long r = s / mx;
+        dst[s] = U[field * P.fstride + (long long)i + (long long)P.px * r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Ghost fill along one axis (A9).  Launched for AXIS = 0, 1, 2 in this order; each later axis sweeps
+// the already-extended range of the earlier ones, so edges and corners are filled.  One thread per
+// (transverse position, side); it writes ghost layers 1 then 2 (layer 2 chains eq. (14) from layer 1).
+//   periodic: copy.   reflecting wall: u_n -> -u_n, T_g = T_src.
+//   fixed-T no-slip wall: u -> -u (all components), T_g = 2 T_w - T_src.
+//   rho_g from the discrete hydrostatic relation (14), PAPER.md:237:
+//       p_g - p_prev = 1/2 (rho_prev + rho_g) delta,  delta = Phi_prev - Phi_g = -+ g_d h,  p_g = rho_g T_g.
+// ------------------------------------------------------------------------------------------------
+template <int AXIS>
+ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
+    // transverse extents (a = faster transverse axis, b = slower one)
+    int na, nb, loa, lob;
+    if (AXIS == 0)      { na = P.ny;            loa = 0;        nb = P.nz;                        lob = 0; }
+    else if (AXIS == 1) { na = P.nx + 2 * ARK_NG; loa = -ARK_NG; nb = P.nz;                        lob = 0; }
+    else                { na = P.nx + 2 * ARK_NG; loa = -ARK_NG; nb = P.ny + 2 * ARK_NG;           lob = -ARK_NG; }
+    const long long ntr = (long long)na * nb;
+    const int n = AXIS == 0 ? P.nx : (AXIS == 1 ? P.ny : P.nz);
+    const long long sd = AXIS == 0 ? 1 : (AXIS == 1 ? (long long)P.px : (long long)P.px * P.py);
+    const double* __restrict__ Uc = U;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < 2 * ntr; s += (long long)gridDim.x * blockDim.x) {
+        const int side = (int)(s / ntr);
+        const long long r = s % ntr;
+        const int a = loa + (int)(r % na), b = lob + (int)(r / na);
+        int c[3];
+        if (AXIS == 0)      { c[0] = 0; c[1] = a; c[2] = b; }
+        else if (AXIS == 1) { c[0] = a; c[1] = 0; c[2] = b; }
+        else                { c[0] = a; c[1] = b; c[2] = 0; }
+        const long long base = ark_idx(P, c[0], c[1], c[2]);     // index of interior cell 0 along AXIS
+        const int type = P.bc[AXIS][side];
+        for (int l = 1; l <= ARK_NG; ++l) {
+            const int ig = side == 0 ? -l : n - 1 + l;
+            const long long jg = base + ig * sd;
+            if (type == ARK_BCK_PERIODIC) {
+                const int is = side == 0 ? n - l : l - 1;
+                const long long js = base + is * sd;
+                for (int f = 0; f < P.nf; ++f) U[f * P.fstride + jg] = Uc[f * P.fstride + js];
+                continue;
+            }
+            const int is = side == 0 ? l - 1 : n - l;             // mirror cell
+            const int ip = side == 0 ? ig + 1 : ig - 1;           // previous cell of the hydrostatic chain
+            const long long js = base + is * sd, jp = base + ip * sd;
+            const long long fE = (long long)(P.nf - 1) * P.fstride;
+            const double mzs = P.ndim == 3 ? U[3 * P.fstride + js] : 0.0;
+            const double mzp = P.ndim == 3 ? U[3 * P.fstride + jp] : 0.0;
+            const ArkPrim ws = ark_prim(P, U[js], U[P.fstride + js], U[2 * P.fstride + js], mzs, U[fE + js]);
+            const ArkPrim wp = ark_prim(P, U[jp], U[P.fstride + jp], U[2 * P.fstride + jp], mzp, U[fE + jp]);
+            double ug[3] = {ws.u, ws.v, ws.w};
+            double Tg;
+            if (type == ARK_BCK_REFLECTING) {
+                ug[AXIS] = -ug[AXIS];
+                Tg = ws.T;
+            } else {
+                ug[0] = -ug[0]; ug[1] = -ug[1]; ug[2] = -ug[2];
+                Tg = 2.0 * P.bcv[AXIS][side] - ws.T;
+            }
+            const double delta = (side == 0 ? -1.0 : 1.0) * P.g[AXIS] * P.h;
+            const double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
+            const double pg = rg * Tg;
+            U[jg] = rg;
+            U[P.fstride + jg] = rg * ug[0];
+            U[2 * P.fstride + jg] = rg * ug[1];
+            if (P.ndim == 3) U[3 * P.fstride + jg] = rg * ug[2];
+            U[fE + jg] = pg / P.gm1 + 0.5 * rg * (ug[0] * ug[0] + ug[1] * ug[1] + ug[2] * ug[2]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// CFL rate of one cell (reading A4):
+//   rate = sum_d (|u_d| + c)/h + 2 ndim max(4 mu/3, (gamma-1) kappa) / (rho h^2)
+// ------------------------------------------------------------------------------------------------
+ARK_DEV double ark_rate(const ArkParams& P, double rho, double mx, double my, double mz, double E,
+                        double inv_h, double dcoef) {
+    const double rinv = 1.0 / rho;
+    const double u = mx * rinv, v = my * rinv, w = mz * rinv;
+    const double p = P.gm1 * (E - 0.5 * (mx * u + my * v + mz * w));
+    const double c = sqrt(P.gamma * p * rinv);
+    const double s = fabs(u) + fabs(v) + (P.ndim == 3 ? fabs(w) : 0.0) + (double)P.ndim * c;
+    return s * inv_h + dcoef * rinv;
+}
+
+// block-wide NaN-propagating max: warp shuffles, then one value per warp through shared memory.
+// Every thread of the block must call it; the result is valid in thread 0.
+ARK_DEV double ark_block_nanmax(double v, double* red /* >= 32 doubles of shared memory */) {
+#ifndef ARK_HOST_EMU
+    for (int o = 16; o > 0; o >>= 1) v = ark_nanmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        v = lane < nw ? red[lane] : -1.0;
+        for (int o = 16; o > 0; o >>= 1) v = ark_nanmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    }
+#else
+    v = ark_emu_block_nanmax(v);
+#endif
+    return v;
+}
+
+// pass 1: grid-stride running max per thread -> one value per block in scratch[blockIdx.x]
+ARK_GLOBAL void ark_k_cfl_pass1(ArkParams P, const double* __restrict__ U, double* __restrict__ scratch) {
+    ARK_SHARED double red[32];
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    const double inv_h = 1.0 / P.h;
+    const double dcoef = 2.0 * P.ndim * fmax(4.0 * P.mu / 3.0, P.gm1 * P.kappa) * inv_h * inv_h;
+    const long long fE = (long long)(P.nf - 1) * P.fstride;
+    double m = -1.0;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(s % P.nx);
+        const long long r = s / P.nx;
+        const long long c = ark_idx(P, i, (int)(r % P.ny), (int)(r / P.ny));
+        const double mz = P.ndim == 3 ? U[3 * P.fstride + c] : 0.0;
+        m = ark_nanmax(m, ark_rate(P, U[c], U[P.fstride + c], U[2 * P.fstride + c], mz, U[fE + c], inv_h, dcoef));
+    }
+    m = ark_block_nanmax(m, red);
+    if (threadIdx.x == 0) scratch[blockIdx.x] = m;
+}
+
+// pass 2: single block over the per-block values; result[0] = max rate,
+// result[1] = dt = cfl / max rate (used by the device-side time loop of ark_run).
+ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, double cfl, double* __restrict__ result,
+                                double* __restrict__ dt_log, int step_index) {
+    ARK_SHARED double red[32];
+    double m = -1.0;
+    for (int s = threadIdx.x; s < nvals; s += blockDim.x) m = ark_nanmax(m, scratch[s]);
+    m = ark_block_nanmax(m, red);
+    if (threadIdx.x == 0) {
+        result[0] = m;
+        result[1] = cfl / m;
+        if (dt_log) dt_log[step_index] = cfl / m;
+    }
+}

@@ -1,0 +1,57 @@
+"""Seeded input generators (paper_1903_09043_b200/inputs.py): determinism, numpy/torch agreement, per-cell
+regeneration of sub-boxes, and the discrete hydrostatic relation (14) of the initial columns."""
+import numpy as np
+import torch
+
+from paper_1903_09043_b200 import inputs as I
+
+
+def test_uniform01_is_counter_based_and_matches_torch():
+    c = np.arange(0, 4096, dtype=np.int64)
+    a = I.uniform01(1234, c)
+    b = I.uniform01(1234, torch.arange(0, 4096, dtype=torch.int64)).numpy()
+    assert np.array_equal(a, b)
+    assert a.min() >= 0.0 and a.max() < 1.0
+    assert abs(a.mean() - 0.5) < 0.02 and abs(a.var() - 1.0 / 12.0) < 0.01
+    assert np.array_equal(I.uniform01(1234, c[100:200]), a[100:200])        # stateless
+    assert not np.array_equal(I.uniform01(1235, c), a)
+    big = I.uniform01(7, np.array([2 ** 40 + 3, 2 ** 62], dtype=np.int64))
+    assert np.all((big >= 0) & (big < 1))
+
+
+def test_torch_and_numpy_builders_agree():
+    for build in (lambda d: I.config1_atmosphere(16, device=d), lambda d: I.config3_rb2d(16, 12, device=d),
+                  lambda d: I.config4_rb3d(8, device=d), lambda d: I.config5_convection3d(8, device=d),
+                  lambda d: I.config2_gresho(16, device=d)):
+        pn, Un = build(None)
+        pt, Ut = build("cpu")
+        assert pn == pt
+        for a, b in zip(Un, Ut):
+            assert (a is None) == (b is None)
+            if a is not None:
+                assert np.array_equal(np.asarray(a).reshape(-1), b.numpy().reshape(-1))
+
+
+def test_sub_box_regeneration():
+    prm, U = I.config5_convection3d(12)
+    box = ((3, 9), (2, 7), (4, 12))
+    prm_b, Ub = I.config5_convection3d(12, box=box)
+    assert prm == prm_b
+    for a, b in zip(U, Ub):
+        assert np.array_equal(a[3:9, 2:7, 4:12], b)
+
+
+def test_columns_satisfy_discrete_hydrostatic_relation():
+    h = 1.0 / 64
+    T, rho = I.polytrope(64, h, 0.57, 0.9, 0.1)
+    p = rho * T
+    lhs = p[1:] - p[:-1]
+    rhs = -0.5 * (rho[1:] + rho[:-1]) * h
+    assert np.abs(lhs - rhs).max() < 1e-15
+    prm, U = I.config5_convection3d(16)
+    assert U[0].max() / U[0].min() > 15          # steep stratification (chi = 100 wall to wall; cell centres see less)
+    assert prm["bc_type"][2] == (I.BC_REFLECTING, I.BC_REFLECTING) and prm["mu"] == 1e-4
+    prm, U = I.config4_rb3d(8)
+    assert abs(prm["mu"] - 7.473e-4) < 2e-6 and abs(prm["kappa"] - 1.8683e-3) < 5e-6
+    prm, U = I.config3_rb2d(16, 8)
+    assert abs(prm["mu"] - 1.8544e-3) < 2e-6 and abs(prm["kappa"] - 4.6361e-3) < 5e-6

@@ -1,0 +1,291 @@
+"""GPU parity: the CUDA path (through the C ABI / thin binding) against the oracle, element by element, on the same
+seeded inputs.  Bar (BASELINE.json north_star): max relative error 1e-11 per field after 10 steps, err_f =
+max|gpu - oracle| / max|oracle| (reading A20); hydrostatic velocities below 1e-12.  The oracle's dt is fed to
+both sides; compute_dt is compared separately (1e-13)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ark_oracle as O
+from paper_1903_09043_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+PER, REF, FIX = I.BC_PERIODIC, I.BC_REFLECTING, I.BC_FIXED_T
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1903_09043_b200 import binding
+    binding.load()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return binding
+
+
+def to_dev(U):
+    return [None if a is None else torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).reshape(-1).cuda() for a in U]
+
+
+def to_np(U):
+    return [None if a is None else a.cpu().numpy() for a in U]
+
+
+def gpu_run(B, prm, U, dts):
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    for dt in dts:
+        s.step(dt)
+    out = to_np(s.get_state())
+    n_launch = s.launch_count()
+    s.close()
+    assert n_launch > 0
+    return out
+
+
+def rel_err(ref, got):
+    e = []
+    for f in range(5):
+        if got[f] is None:
+            e.append(0.0)
+            continue
+        scale = np.abs(ref[f]).max()
+        e.append(float(np.abs(ref[f] - got[f]).max() / scale) if scale > 0 else float(np.abs(got[f]).max()))
+    return e
+
+
+# the five BASELINE configs at sizes the oracle finishes in seconds; every grid spans several 32x8 tiles and has a
+# ragged tail in x and/or y (sizes not multiples of the tile) and, in 3D, several z chunks
+CONFIGS = {
+    "config1_atmosphere_128": lambda: I.config1_atmosphere(128),
+    "config1_atmosphere_theta_off_100": lambda: I.config1_atmosphere(100, theta=0),
+    "config2_gresho_150": lambda: I.config2_gresho(150),
+    "config2_gresho_theta_off_96": lambda: I.config2_gresho(96, theta=0),
+    "config3_rb2d_200x100": lambda: I.config3_rb2d(200, 100),
+    "config4_rb3d_72": lambda: I.config4_rb3d(72),
+    "config5_convection3d_80": lambda: I.config5_convection3d(80),
+    "config5_mach_half_noise_48": lambda: I.config5_convection3d(48, amp=0.05),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CONFIGS))
+def test_parity_10_steps(B, name):
+    prm, U = CONFIGS[name]()
+    ref, dts = O.run(prm, U, 10, cfl=0.4)
+    got = gpu_run(B, prm, U, dts)
+    err = rel_err(ref, got)
+    assert max(err) < TOL, (name, err)
+
+
+RANDOM = {
+    "2d_periodic": lambda: I.random_state(70, 37, 1, 3),
+    "2d_walls_gravity_viscous": lambda: I.random_state(67, 45, 1, 4, mu=2e-3, kappa=3e-3, g=(0, -1.0, 0),
+                                                       bc_type=((PER, PER), (FIX, REF), (0, 0)), bc_value=((0, 0), (2.5, 0), (0, 0))),
+    "2d_gravity_x": lambda: I.random_state(40, 33, 1, 14, g=(-0.7, 0.3, 0), bc_type=((REF, REF), (REF, REF), (0, 0))),
+    "3d_periodic": lambda: I.random_state(45, 21, 19, 5),
+    "3d_walls_viscous": lambda: I.random_state(37, 26, 40, 6, mu=2e-3, kappa=3e-3, g=(0, 0, -1.0),
+                                               bc_type=((PER, PER), (PER, PER), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))),
+    "3d_all_walls_oblique": lambda: I.random_state(33, 10, 18, 7, mu=1e-3, kappa=0.0, g=(0.2, -0.3, -1.0),
+                                                   bc_type=((REF, FIX), (FIX, REF), (REF, REF)), bc_value=((0, 2.5), (2.2, 0), (0, 0))),
+    "3d_minimum_size": lambda: I.random_state(4, 4, 4, 8, mu=1e-3, kappa=1e-3),
+    "2d_minimum_size": lambda: I.random_state(4, 4, 1, 9),
+}
+
+
+@pytest.mark.parametrize("name", sorted(RANDOM))
+def test_parity_random_states(B, name):
+    """O(1) random states (strong gradients, all upwind directions, theta saturating at 1): 5 steps, 1e-12."""
+    prm, U = RANDOM[name]()
+    ref, dts = O.run(prm, U, 5, cfl=0.4)
+    got = gpu_run(B, prm, U, dts)
+    err = rel_err(ref, got)
+    assert max(err) < 1e-12, (name, err)
+
+
+def test_hydrostatic_atmosphere_stays_at_rest(B):
+    """north_star: hydrostatic velocities below 1e-12 (unperturbed config 1 and the conductive polytropes)."""
+    cases = [I.config1_atmosphere(128, amp=0.0), I.config1_atmosphere(128, amp=0.0, theta=0),
+             I.config3_rb2d(64, 96, amp=0.0), I.config4_rb3d(40, amp=0.0), I.config5_convection3d(40, amp=0.0)]
+    for prm, U in cases:
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        s.run(300, 0.4)
+        out = to_np(s.get_state())
+        s.close()
+        vmax = max(np.abs(out[f] / out[0]).max() for f in (1, 2, 3) if out[f] is not None)
+        assert vmax < 1e-12, (prm["nx"], prm["nz"], vmax)
+        assert np.abs(out[0] - np.asarray(U[0]).reshape(-1)).max() < 1e-11 * np.abs(out[0]).max()
+
+
+def test_uniform_state_is_bit_exact(B):
+    for shape in ((1, 20, 40), (12, 20, 40)):
+        nz, ny, nx = shape
+        prm = I.make_params(nx, ny, nz, 0.1, 1.4, mu=0.01, kappa=0.02)
+        rho, u, v, w, p = 1.25, 0.5, -0.25, (0.125 if nz > 1 else 0.0), 0.75
+        E = p / 0.4 + 0.5 * rho * (u * u + v * v + w * w)
+        U = [np.full(shape, x) for x in (rho, rho * u, rho * v, rho * w, E)]
+        if nz == 1:
+            U[3] = None
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        s.run(5, 0.4)
+        out = to_np(s.get_state())
+        s.close()
+        for f in range(5):
+            if out[f] is not None:
+                assert np.array_equal(out[f], U[f].reshape(-1)), f
+
+
+def test_ghost_fill_matches_oracle(B):
+    for name in ("2d_walls_gravity_viscous", "3d_all_walls_oblique", "3d_periodic", "2d_gravity_x"):
+        prm, U = RANDOM[name]()
+        ref = O.fill_ghosts(prm, U)
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        got = to_np(s.get_padded())
+        s.close()
+        for f in range(5):
+            if got[f] is None:
+                continue
+            assert np.abs(got[f] - ref[f]).max() <= 4e-15 * np.abs(ref[f]).max(), (name, f)
+    # periodic ghost fill is a pure copy: bit exact
+    prm, U = RANDOM["3d_periodic"]()
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    got = to_np(s.get_padded())
+    s.close()
+    for f in range(5):
+        assert np.array_equal(got[f], np.pad(U[f], 2, mode="wrap"))
+
+
+def test_compute_dt_and_run_match_oracle(B):
+    for name in ("2d_walls_gravity_viscous", "3d_walls_viscous", "3d_periodic"):
+        prm, U = RANDOM[name]()
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        dt0 = s.compute_dt(0.4)
+        assert abs(dt0 - O.compute_dt(prm, U, 0.4)) <= 1e-13 * dt0          # standalone two-pass reduction
+        ref, dts = O.run(prm, U, 6, cfl=0.4)
+        got_dts = []
+        for i in range(3):                                                   # host loop: compute_dt + step
+            dt = s.compute_dt(0.4)                                           # steps 2,3 use the fused epilogue's rates
+            got_dts.append(dt)
+            s.step(dt)
+        got_dts += s.run(3, 0.4, want_dts=True)                              # device-side loop
+        out = to_np(s.get_state())
+        s.close()
+        assert np.abs(np.array(got_dts) - dts).max() <= 1e-12 * dts.max(), (got_dts, dts)
+        assert max(rel_err(ref, out)) < 1e-12
+
+
+def test_set_get_roundtrip_device_and_host(B):
+    prm, U = RANDOM["3d_walls_viscous"]()
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    out = to_np(s.get_state())
+    for f in range(5):
+        assert np.array_equal(out[f], U[f].reshape(-1))
+    host_in = [torch.as_tensor(np.ascontiguousarray(a)).reshape(-1).pin_memory() for a in U]
+    s.set_state_host(host_in)
+    host_out = [torch.empty_like(a).pin_memory() for a in host_in]
+    s.get_state_host(host_out)
+    for f in range(5):
+        assert np.array_equal(host_out[f].numpy(), U[f].reshape(-1))
+    s.close()
+    prm, U = RANDOM["2d_periodic"]()
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    out = to_np(s.get_state())
+    assert out[3] is None
+    for f in (0, 1, 2, 4):
+        assert np.array_equal(out[f], U[f].reshape(-1))
+    s.close()
+
+
+def test_nonfinite_state_is_reported(B):
+    prm, U = RANDOM["2d_periodic"]()
+    U = [None if a is None else a.copy() for a in U]
+    U[4][0, 5, 7] = -3.0                                   # negative pressure
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    with pytest.raises(B.ArkError) as ei:
+        s.compute_dt(0.4)
+    assert ei.value.code == B.ARK_ENONFINITE
+    s.close()
+    # blow-up detected through the fused epilogue as well: a huge dt makes the next rate non-finite
+    prm, U = RANDOM["3d_periodic"]()
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    s.step(10.0)
+    with pytest.raises(B.ArkError) as ei:
+        s.compute_dt(0.4)
+    assert ei.value.code == B.ARK_ENONFINITE
+    s.close()
+
+
+def test_conservation_on_gpu(B):
+    """Flux form: mass, transverse momentum and E + rho*Phi conserved to round-off by the CUDA path itself."""
+    prm, U = I.random_state(64, 48, 40, 10, g=(0, 0, -2.0), mu=1e-3, kappa=2e-3, bc_type=((PER, PER), (PER, PER), (REF, REF)))
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    s.run(20, 0.4)
+    out = to_np(s.get_state())
+    s.close()
+    k = np.arange(40)[:, None, None]
+    Phi = (2.0 * (k + 0.5) * prm["dx"] + 0 * U[0]).reshape(-1)
+    import math
+    m0, m1 = math.fsum(U[0].reshape(-1)), math.fsum(out[0])
+    e0 = math.fsum(U[4].reshape(-1) + U[0].reshape(-1) * Phi)
+    e1 = math.fsum(out[4] + out[0] * Phi)
+    assert abs(m1 - m0) < 1e-13 * m0 and abs(e1 - e0) < 1e-13 * abs(e0)
+
+
+@pytest.mark.parametrize("cfg", ["config4_256", "config5_512"])
+def test_full_size_sampled_parity(B, cfg):
+    """BASELINE full sizes, the launch configuration bench.py times.  One step of U^{n+1} depends on U^n within
+    2 cells, so the oracle recomputes sampled sub-boxes (interior, x/y periodic seams, both z walls) from the
+    same counter-based inputs and must agree with the GPU's full-size result there."""
+    if cfg == "config4_256":
+        n, build = 256, I.config4_rb3d
+    else:
+        n, build = 512, I.config5_convection3d
+        free, _ = torch.cuda.mem_get_info()
+        if free < 40e9:
+            pytest.skip("not enough device memory for 512^3")
+    prm, U = build(n, device="cuda")
+    U = [a.reshape(-1) for a in U]
+    s = B.Solver(prm)
+    s.set_state(U)
+    dt = s.compute_dt(0.4)
+    s.step(dt)
+    out = [a.reshape(n, n, n) for a in s.get_state()]
+    dt2 = s.compute_dt(0.4)                      # from the fused epilogue
+    assert 0.5 * dt < dt2 < 2.0 * dt
+    s.close()
+    W = 12                                       # compared box edge; oracle runs on W+4 with 2 sacrificial cells per cut side
+    rng = np.random.RandomState(0)
+    boxes = [(0, 0, 0), (n - W, n - W, n - W), (0, 100, n - W), (n - W, 0, 37), (n // 2 - 3, n // 2 + 5, n // 2)]
+    boxes += [tuple(int(v) for v in rng.randint(0, n - W, 3)) for _ in range(3)]
+    for (k0, j0, i0) in boxes:
+        # sub-box with a 2-cell margin where the domain continues (periodic x/y wrap handled by modular indices)
+        lo_wall, hi_wall = k0 == 0, k0 + W == n
+        ka, kb = (k0 if lo_wall else k0 - 2), (k0 + W if hi_wall else k0 + W + 2)
+        jj = np.arange(j0 - 2, j0 + W + 2) % n
+        ii = np.arange(i0 - 2, i0 + W + 2) % n
+        sub = []
+        for f in range(5):
+            full = U[f].reshape(n, n, n)
+            blk = full[ka:kb][:, torch.as_tensor(jj, device="cuda")][:, :, torch.as_tensor(ii, device="cuda")]
+            sub.append(blk.cpu().numpy())
+        wall = prm["bc_type"][2][0]
+        bt = ((PER, PER), (PER, PER), (wall if lo_wall else REF, wall if hi_wall else REF))
+        if not lo_wall and not hi_wall:
+            bt = ((PER, PER), (PER, PER), (REF, REF))
+        prm_b = dict(prm, nx=W + 4, ny=W + 4, nz=kb - ka, bc_type=bt)
+        ref, _ = O.run(prm_b, sub, 1, dts=[dt])
+        zs = slice(0 if lo_wall else 2, (kb - ka) if hi_wall else (kb - ka - 2))
+        for f in range(5):
+            r = ref[f].reshape(kb - ka, W + 4, W + 4)[zs, 2:-2, 2:-2]
+            g = out[f][k0:k0 + W, j0:j0 + W, i0:i0 + W].cpu().numpy()
+            scale = np.abs(r).max()
+            assert np.abs(r - g).max() <= 1e-12 * scale, (cfg, (k0, j0, i0), f, np.abs(r - g).max(), scale)
