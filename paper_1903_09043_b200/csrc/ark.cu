@@ -53,7 +53,7 @@ Layout make_layout(int nx, int ny, int nz) {
     const bool d3 = nz > 1;
     L.nf = d3 ? 5 : 4;
     L.offz = d3 ? ARK_NG : 0;
-    L.px = (int)round_up((size_t)nx + 2 * ARK_NG, 16);
+    L.px = (int)round_up((size_t)nx + ARK_XOFF + ARK_NG, 16);
     L.py = ny + 2 * ARK_NG;
     L.pz = d3 ? nz + 2 * ARK_NG : 1;
     L.fstride = (long long)round_up((size_t)L.px * L.py * L.pz, 32);

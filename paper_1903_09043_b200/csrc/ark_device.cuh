@@ -4,8 +4,10 @@
 // This file shares nothing with oracle/: every formula is restated here from the paper.
 //
 // HBM layout: SoA fp64, one padded array per conserved field (rho, rho*u, rho*v, [rho*w], E),
-// 2 ghost layers per side (A9), x fastest, row pitch px (multiple of 16 doubles = 128 B), so the
-// halo'd tile of a block starts on a 128-byte boundary whenever the tile origin is a multiple of 16.
+// 2 ghost layers per side (A9), x fastest, row pitch px (multiple of 16 doubles = 128 B).  Interior cell
+// i = 0 sits at x index ARK_XOFF = 4 of a row (2 unused doubles, then the 2 low ghosts), so that the
+// 28-wide output rows of the step kernel (tile origin a multiple of 28 = 7 sectors) start on a 32-byte
+// sector boundary and every store of the hot kernel writes whole sectors.
 #pragma once
 
 #ifndef ARK_HOST_EMU
@@ -21,6 +23,7 @@
 
 #define ARK_K_IMPEDANCE 1.1  // a = K max(rho_L c_L, rho_R c_R), reading A2
 #define ARK_NG 2             // ghost layers (A9)
+#define ARK_XOFF 4           // x index of interior cell 0 inside a padded row (>= ARK_NG)
 
 enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2 };
 
@@ -37,11 +40,20 @@ struct ArkParams {
 
 // padded linear index of interior-based cell (i,j,k); ghosts are -2,-1 and n,n+1
 ARK_DEV long long ark_idx(const ArkParams& P, int i, int j, int k) {
-    return (long long)(i + ARK_NG) + (long long)P.px * ((long long)(j + ARK_NG) + (long long)P.py * (long long)(k + P.offz));
+    return (long long)(i + ARK_XOFF) + (long long)P.px * ((long long)(j + ARK_NG) + (long long)P.py * (long long)(k + P.offz));
 }
 
 // NaN-propagating max (fmax would drop NaNs): SURVEY 8(a) row 8
 ARK_DEV double ark_nanmax(double a, double b) { return (a != a) ? a : ((b != b) ? b : (a > b ? a : b)); }
+
+// The same for values that are >= 0 when valid (CFL rates), on the integer pipe: for non-negative doubles the
+// IEEE-754 bit pattern is monotone as an unsigned integer, every NaN and every negative value compares above
+// +inf, so an unsigned max keeps the largest rate and lets any invalid value win (it is then reported as
+// non-finite / non-positive by the caller).  Keeps DSETP traffic off the fp64 pipe in the step kernel.
+typedef unsigned long long ark_u64;
+ARK_DEV ark_u64 ark_rate_bits(double r) { return (ark_u64)__double_as_longlong(r); }
+ARK_DEV double ark_rate_from_bits(ark_u64 b) { return __longlong_as_double((long long)b); }
+ARK_DEV ark_u64 ark_umax(ark_u64 a, ark_u64 b) { return a > b ? a : b; }
 
 // ------------------------------------------------------------------------------------------------
 // Primitive variables of one cell (PAPER.md:315-319 ideal gas, c^2 = gamma p / rho; :370 p = rho T).
@@ -77,14 +89,17 @@ ARK_DEV ArkFace ark_face(int theta_on, double gh,
                          double rhoL, double unL, double pL, double rcL, double ircL,
                          double rhoR, double unR, double pR, double rcR, double ircR) {
     ArkFace f;
-    const double a = ARK_K_IMPEDANCE * fmax(rcL, rcR);
-    const double i2a = (0.5 / ARK_K_IMPEDANCE) * fmin(ircL, ircR);
+    // one comparison picks max(rc) and min(1/rc) (plain selects: fmax/fmin on doubles cost ~6 instructions)
+    const bool lg = rcL > rcR;
+    const double a = ARK_K_IMPEDANCE * (lg ? rcL : rcR);
+    const double i2a = (0.5 / ARK_K_IMPEDANCE) * (lg ? ircL : ircR);
     f.S = (0.5 * gh) * (rhoL + rhoR);
     f.us = 0.5 * (unL + unR) - ((pR - pL) - f.S) * i2a;
     double ath = a;
     if (theta_on) {
-        const double icm = fmin(rhoL * ircL, rhoR * ircR);
-        ath = a * fmin(fabs(f.us) * icm, 1.0);
+        const double icL = rhoL * ircL, icR = rhoR * ircR;          // 1/c
+        const double ma = fabs(f.us) * (icL < icR ? icL : icR);     // |u*| / max(c_L, c_R)
+        ath = a * (ma < 1.0 ? ma : 1.0);
     }
     f.pi = 0.5 * (pL + pR) - 0.5 * ath * (unR - unL);
     return f;
@@ -120,7 +135,7 @@ ARK_GLOBAL void ark_k_unpack_padded(ArkParams P, const double* __restrict__ U, d
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(s % mx);
         const long long r = s / mx;
-        dst[s] = U[field * P.fstride + (long long)i + (long long)P.px * r];
+        dst[s] = U[field * P.fstride + (long long)(i + ARK_XOFF - ARK_NG) + (long long)P.px * r];
     }
 }
 

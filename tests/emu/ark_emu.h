@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <barrier>
 #include <cmath>
+#include <cstring>
 #include <functional>
 #include <memory>
 #include <thread>
@@ -25,6 +26,8 @@ inline std::vector<double> ark_emu_red;
 #define __syncthreads() ark_emu_barrier->arrive_and_wait()
 
 inline double rsqrt(double x) { return 1.0 / std::sqrt(x); }
+inline long long __double_as_longlong(double x) { long long r; std::memcpy(&r, &x, 8); return r; }
+inline double __longlong_as_double(long long x) { double r; std::memcpy(&r, &x, 8); return r; }
 
 inline double ark_emu_block_nanmax(double v) {
     ark_emu_red[threadIdx.x] = v;
@@ -39,11 +42,22 @@ inline double ark_emu_block_nanmax(double v) {
     return v;
 }
 
+inline std::vector<unsigned long long> ark_emu_redu;
+inline unsigned long long ark_emu_block_umax(unsigned long long v) {
+    ark_emu_redu[threadIdx.x] = v;
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (unsigned i = 1; i < blockDim.x; ++i) v = std::max(v, ark_emu_redu[i]);
+    __syncthreads();
+    return v;
+}
+
 // run f() for every thread of every block of the grid
 inline void ark_emu_launch(emu_dim3 grid, unsigned nthreads, size_t smem_bytes, const std::function<void()>& f) {
     std::vector<double> smem(smem_bytes / sizeof(double) + 1);
     ark_emu_smem = smem.data();
     ark_emu_red.assign(nthreads, 0.0);
+    ark_emu_redu.assign(nthreads, 0ULL);
     for (unsigned bz = 0; bz < grid.z; ++bz)
         for (unsigned by = 0; by < grid.y; ++by)
             for (unsigned bx = 0; bx < grid.x; ++bx) {

@@ -16,7 +16,7 @@ ArkParams make_params(int nx, int ny, int nz, double h, double gamma, const doub
     ArkParams P;
     std::memset(&P, 0, sizeof P);
     P.nx = nx; P.ny = ny; P.nz = nz; P.ndim = nz > 1 ? 3 : 2; P.nf = nz > 1 ? 5 : 4;
-    P.px = (nx + 4 + 15) / 16 * 16; P.py = ny + 4; P.pz = nz > 1 ? nz + 4 : 1; P.offz = nz > 1 ? 2 : 0;
+    P.px = (nx + ARK_XOFF + ARK_NG + 15) / 16 * 16; P.py = ny + 4; P.pz = nz > 1 ? nz + 4 : 1; P.offz = nz > 1 ? 2 : 0;
     P.fstride = ((long long)P.px * P.py * P.pz + 31) / 32 * 32;
     P.h = h; P.gamma = gamma; P.gm1 = gamma - 1.0; P.mu = mu; P.kappa = kappa; P.theta = theta;
     for (int d = 0; d < 3; ++d) {
@@ -78,7 +78,7 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
             for (int f = 0; f < P.nf; ++f)
                 for (long long r = 0; r < (long long)P.py * P.pz; ++r)
                     for (int i = 0; i < mx; ++i)
-                        padded_out[(size_t)f * mx * P.py * P.pz + r * mx + i] = cur[f * P.fstride + r * P.px + i];
+                        padded_out[(size_t)f * mx * P.py * P.pz + r * mx + i] = cur[f * P.fstride + r * P.px + i + (ARK_XOFF - ARK_NG)];
         }
         if (P.ndim == 3) { if (visc) step<3, true>(P, cur, nxt, dts[s], scratch.data(), zchunk, grid); else step<3, false>(P, cur, nxt, dts[s], scratch.data(), zchunk, grid); }
         else             { if (visc) step<2, true>(P, cur, nxt, dts[s], scratch.data(), zchunk, grid); else step<2, false>(P, cur, nxt, dts[s], scratch.data(), zchunk, grid); }
