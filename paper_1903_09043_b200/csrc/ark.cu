@@ -102,7 +102,7 @@ int grid_for(long long n, int block, int cap = 148 * 8) {
 
 template <int NDIM, bool VISC, int TX, int TY>
 int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
-    using C = ArkStepCfg<TX, TY>;
+    using C = ArkStepCfg<NDIM, VISC, TX, TY>;
     static bool attr_set = false;
     auto kern = ark_k_step<NDIM, VISC, TX, TY>;
     if (!attr_set) {

@@ -6,41 +6,57 @@
 //
 // Decomposition ("2.5-D marching"): a block owns a TX x TY tile of (x,y) columns plus a 2-cell halo
 // (region RX x RY = (TX+4) x (TY+4), one thread per column) and marches along z over a chunk of planes.
-// The product build uses TX = 28, so RX = 32: ONE WARP PER REGION ROW.  Every role that depends on the
-// row (halo row / ring row / output row) is then warp-uniform -- halo warps skip whole phases instead of
-// idling lanes -- and every global load of a warp is one contiguous 256-byte row segment.
+// The product build uses TX = 28, so RX = 32: ONE WARP PER REGION ROW.  Every role in the kernel depends on
+// the ROW only (halo row / ring row / output row), i.e. is warp-uniform: halo warps skip whole phases, no
+// lane is predicated off inside a phase (the 4 halo lanes of a row compute values nobody consumes), and every
+// global access of a warp is one contiguous 256-byte row segment.  Only the final stores and the CFL rate
+// carry a per-lane predicate.
+//
+// What persists from plane to plane lives in shared memory rings owned by the column's thread --
+//   UR  U^n of planes q, q+1, q+2   (filled by 8-byte cp.async two planes ahead: the HBM prefetch costs no
+//                                    registers and no instructions on the critical path)
+//   PB  primitives of planes q-1, q, q+1 (x/y neighbours read them; the own column's z neighbours too)
+//   TB  U~ of planes q-1, q
+// -- so the register pipeline along z is only the running update acc[5], the low z face and four velocity
+// differences, and nothing has to be rotated through registers at the end of an iteration.
 //
 // Per plane q one iteration does (3 block barriers):
-//   S1  primitives of plane q+1 (own column, from registers)           -> smem PB (2-plane ring)
+//   S1  primitives of plane q+1 (own column, from the UR ring)          -> PB
 //   --- barrier A
-//   S2  acoustic faces x-, y- of plane q (neighbours from PB), z face (q|q+1) from registers   -> smem FB
-//       cell-centred velocity differences of plane q (x,y neighbours from PB, z from registers) -> smem GB
+//   S2  acoustic faces x-, y- of plane q (neighbours from PB), z face (q|q+1) from the own column   -> FB
+//       cell-centred velocity differences of plane q                                               -> GB
 //   --- barrier B
-//   S3  acoustic update U~(q) on tile + 1 ring       -> smem TB
-//       viscous / heat fluxes through the x-, y- faces of plane q      -> smem VB ; z- face in registers
+//   S3  acoustic update U~(q) on tile + 1 ring       -> TB
+//       viscous / heat fluxes through the x-, y- faces of plane q      -> VB ; z- face in registers
 //   --- barrier C
 //   S4  transport fluxes (upwind on u*) of the in-plane faces of plane q and of the
 //       z face (q-1|q); completes and stores U^{n+1}(q-1); folds the CFL rate of the new state into a
 //       per-block maximum (integer max on the bit patterns, NaN-propagating).
-// z neighbours of a column stay in the owning thread's registers; only x/y neighbours go through
-// shared memory.
 #pragma once
 #include "ark_device.cuh"
 
 #define ARK_NPRIM 8   // rho,u,v,w,p,rc,irc,T
 
-template <int TX, int TY>
+template <int NDIM, bool VISC, int TX, int TY>
 struct ArkStepCfg {
     static constexpr int RX = TX + 4, RY = TY + 4, NCOL = RX * RY;
     static constexpr int NT = ((NCOL + 31) / 32) * 32;
-    // shared memory (doubles per column): PB[2][8] FB[6] GB[7] TB[5] VB[8]  (+ 32 for the block reduction)
-    static constexpr int PER_COL = 2 * ARK_NPRIM + 6 + 7 + 5 + 8;
+    static constexpr int NP = VISC ? 8 : 7;                          // T only feeds the heat flux
+    static constexpr int PSLOTS = NDIM == 3 ? (VISC ? 3 : 2) : 1;    // plane q-1 only feeds the viscous z stencil
+    static constexpr int UR = NDIM == 3 ? 15 : 0;                    // [3][5]
+    static constexpr int TSLOTS = NDIM == 3 ? 2 : 1;
+    // shared memory (doubles per column): UR, PB[PSLOTS][NP], FB[6], TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
+    static constexpr int PER_COL = UR + PSLOTS * NP + 6 + TSLOTS * 5 + (VISC ? 15 : 0);
     static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32;
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
 };
 
-// cheap two-way selects (fmax/fmin on doubles expand to DSETP + FSEL/SEL + NaN quieting + moves)
-ARK_DEV double ark_sel(bool c, double a, double b) { return c ? a : b; }
+// sign tests on the integer pipe (the fp64 pipe is the bottleneck of this kernel): for u* >= 0 the paper's
+// upwind choice is the left cell (reading A10); -0.0 picks the right cell, whose flux is
+// multiplied by that same zero.
+ARK_DEV bool ark_nonneg(double x) { return (int)(__double_as_longlong(x) >> 32) >= 0; }
+ARK_DEV double ark_pos_part(double x) { return ark_nonneg(x) ? x : 0.0; }   // max(x, 0)
+ARK_DEV double ark_neg_part(double x) { return ark_nonneg(x) ? 0.0 : x; }   // min(x, 0)
 
 // Coefficients of the dissipative face flux, precomputed once per thread.
 struct ArkViscCoef { double cn, ct, c43, c23t, kh; };
@@ -70,70 +86,98 @@ ARK_DEV ArkVisc ark_visc_face(const ArkViscCoef& K, double dn_n, double dn_a, do
 }
 
 // CFL rate of one cell of the NEW state for the fused epilogue (reading A4), as the bit pattern of |rate|
-// (see ark_rate_bits): one reciprocal and one square root per cell.
+// (see ark_rate_bits): one fast reciprocal and one fast rsqrt per cell.
 ARK_DEV ark_u64 ark_rate_epilogue(const ArkParams& P, int ndim, double rho, double mx, double my, double mz, double E,
                                   double inv_h, double dcoef) {
-    const double rinv = 1.0 / rho;
+    const double rinv = ark_rcp(rho);
     const double s = (fabs(mx) + fabs(my) + fabs(mz)) * rinv;
     const double ke = 0.5 * (mx * mx + my * my + mz * mz) * rinv;
-    const double c = sqrt(P.gamma * (P.gm1 * (E - ke)) * rinv);
+    const double c2 = P.gamma * (P.gm1 * (E - ke)) * rinv;
+    const double c = c2 * ark_rsqrt(c2);
     const double r = (s + (double)ndim * c) * inv_h + dcoef * rinv;
     return ark_rate_bits(r) & 0x7fffffffffffffffULL;
 }
 
-template <int NDIM, bool VISC, int TX, int TY>
-ARK_GLOBAL void
-#ifndef ARK_HOST_EMU
-__launch_bounds__(ArkStepCfg<TX, TY>::NT, 1)
-#endif
-ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict__ Uout,
-           double dt_value, const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk) {
-    using C = ArkStepCfg<TX, TY>;
-    constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL;
-    constexpr int NF = NDIM == 3 ? 5 : 4;
-    constexpr int FE = NF - 1;                        // index of the energy field in HBM
-    ARK_DYN_SMEM(smem);
-    double* PB = smem;                                // [2][NPRIM][NCOL]
-    double* FB = PB + 2 * ARK_NPRIM * NCOL;           // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
-    double* GB = FB + 6 * NCOL;                       // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (centred differences)
-    double* TB = GB + 7 * NCOL;                       // [5][NCOL]: U~(q)
-    double* VB = TB + 5 * NCOL;                       // [8][NCOL]: viscous low-face fluxes x(4), y(4)
-    ark_u64* red = (ark_u64*)(VB + 8 * NCOL);         // [32]
+// per-thread constants of a step
+struct ArkStepConst {
+    double dt, lam, inv_h, ghx, ghy, ghz, dcoef;
+    bool gx_on, gy_on, gz_on;
+    int th;
+    ArkViscCoef KV;
+};
+
+ARK_DEV ArkStepConst ark_step_const(const ArkParams& P, double dt_value, const double* __restrict__ dt_dev) {
+    ArkStepConst c;
+    c.dt = dt_dev ? dt_dev[1] : dt_value;
+    c.inv_h = 1.0 / P.h;
+    c.lam = c.dt / P.h;
+    c.ghx = P.g[0] * P.h; c.ghy = P.g[1] * P.h; c.ghz = P.g[2] * P.h;
+    c.gx_on = c.ghx != 0.0; c.gy_on = c.ghy != 0.0; c.gz_on = c.ghz != 0.0;
+    c.th = P.theta;
+    c.dcoef = 2.0 * P.ndim * fmax(4.0 * P.mu / 3.0, P.gm1 * P.kappa) * c.inv_h * c.inv_h;
+    c.KV.cn = P.mu * c.inv_h; c.KV.ct = 0.25 * P.mu * c.inv_h; c.KV.c43 = (4.0 / 3.0) * P.mu * c.inv_h;
+    c.KV.c23t = (2.0 / 3.0) * 0.25 * P.mu * c.inv_h; c.KV.kh = P.kappa * c.inv_h;
+    return c;
+}
+
+// Transport through the two faces of one in-plane axis of the cell in column tc (stride sd between neighbours):
+// F = U~_up u* + (0, Pi* e_d, Pi* u*); adds F_{d+} - F_{d-} to dG and the gravity
+// work g_d (min(m_{d+},0) + max(m_{d-},0)) to work (reading A13).  T points at U~ of plane q,
+// component stride cs.  DN = index of the normal momentum (1: x, 2: y).
+template <int NDIM, int DN>
+ARK_DEV void ark_transport_axis(const double* __restrict__ T, int cs, int tc, int sd, double usl, double pil, double ush,
+                                double pih, bool g_on, double g, double* dG, double& work, bool first) {
+    const int nl = ark_nonneg(usl) ? tc - sd : tc, nh = ark_nonneg(ush) ? tc : tc + sd;
+    const double ml = T[nl] * usl, mh = T[nh] * ush;
+    // each face flux is formed first (normal momentum: U~_up u* + Pi*), then differenced: the order of the flux
+    // form (11), which keeps the O(1) pressure terms bit-compatible with a plain evaluation (reading A20)
+    double d[5];
+    d[0] = mh - ml;
+    d[1] = DN == 1 ? (T[cs + nh] * ush + pih) - (T[cs + nl] * usl + pil) : T[cs + nh] * ush - T[cs + nl] * usl;
+    d[2] = DN == 2 ? (T[2 * cs + nh] * ush + pih) - (T[2 * cs + nl] * usl + pil) : T[2 * cs + nh] * ush - T[2 * cs + nl] * usl;
+    d[3] = NDIM == 3 ? T[3 * cs + nh] * ush - T[3 * cs + nl] * usl : 0.0;
+    d[4] = (T[4 * cs + nh] + pih) * ush - (T[4 * cs + nl] + pil) * usl;
+    if (first) { for (int f = 0; f < 5; ++f) dG[f] = d[f]; }
+    else       { for (int f = 0; f < 5; ++f) dG[f] += d[f]; }
+    if (g_on) work += g * (ark_pos_part(ml) + ark_neg_part(mh));
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// 3D body
+// ------------------------------------------------------------------------------------------------------------
+template <bool VISC, int TX, int TY>
+ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
+                        const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem) {
+    using C = ArkStepCfg<3, VISC, TX, TY>;
+    constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP, PSLOTS = C::PSLOTS;
+    double* UR = smem;                                // [3][5][NCOL]
+    double* PB = UR + 15 * NCOL;                      // [PSLOTS][NP][NCOL]
+    double* FB = PB + PSLOTS * NP * NCOL;             // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
+    double* TB = FB + 6 * NCOL;                       // [2][5][NCOL]: U~ of planes q-1, q
+    double* GB = TB + 10 * NCOL;                      // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
+    double* VB = GB + (VISC ? 7 : 0) * NCOL;          // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
+    ark_u64* red = (ark_u64*)(VB + (VISC ? 8 : 0) * NCOL);   // [32]
 
     const int t = threadIdx.x;
-    const bool live = t < NCOL;
-    const int tc = live ? t : NCOL - 1;
+    const int tc = t < NCOL ? t : NCOL - 1;
     const int ci = tc % RX, cj = tc / RX;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
     const int gi = x0 - 2 + ci, gj = y0 - 2 + cj;      // interior-based cell coordinates of this column
-    // clamp columns that fall outside the padded array (ragged tiles): they load a valid cell, results unused
+    // columns beyond the padded array (ragged tiles) load a valid cell; nobody consumes their results
     const int li = gi < P.nx + 2 ? gi : P.nx + 1;
     const int lj = gj < P.ny + 2 ? gj : P.ny + 1;
+    const int k0 = blockIdx.z * zchunk;
+    const int k1 = k0 + zchunk < P.nz ? k0 + zchunk : P.nz;
 
-    const int k0 = NDIM == 3 ? blockIdx.z * zchunk : 0;
-    const int k1 = NDIM == 3 ? (k0 + zchunk < P.nz ? k0 + zchunk : P.nz) : 1;
+    // roles: functions of the row only (warp-uniform when RX == 32)
+    const bool rowF = cj >= 1;                      // owns a low-y face
+    const bool rowA = cj >= 1 && cj <= RY - 2;      // tile + 1 ring: U~, centred differences
+    const bool rowU = cj >= 2 && cj <= RY - 3;      // tile: update
+    const bool rowVy = cj >= 2 && cj <= RY - 2;     // owns a viscous low-y face of the tile
+    const bool inU = t < NCOL && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;   // stores / rate only
 
-    // roles (row conditions are warp-uniform when RX == 32)
-    const bool rowA = cj >= 1 && cj <= RY - 2;                           // tile + 1 ring
-    const bool rowU = cj >= 2 && cj <= RY - 3;                           // tile
-    const bool colA = ci >= 1 && ci <= RX - 2;
-    const bool inFx = live && rowA && ci >= 1;                           // owns the low-x face (ci-1 | ci)
-    const bool inFy = live && cj >= 1 && colA;                           // owns the low-y face (cj-1 | cj)
-    const bool inA = live && rowA && colA && gi <= P.nx && gj <= P.ny;   // acoustic update / centred differences
-    const bool inU = live && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;
-    const bool inVx = VISC && live && rowU && ci >= 2 && ci <= 2 + TX;
-    const bool inVy = VISC && live && cj >= 2 && cj <= 2 + TY && ci >= 2 && ci < 2 + TX;
-
-    const double dt = dt_dev ? dt_dev[1] : dt_value;
-    const double inv_h = 1.0 / P.h;
-    const double lam = dt / P.h;
-    const double ghx = P.g[0] * P.h, ghy = P.g[1] * P.h, ghz = P.g[2] * P.h;
-    const bool gx_on = ghx != 0.0, gy_on = ghy != 0.0;
-    const int th = P.theta;
-    const double dcoef = 2.0 * P.ndim * fmax(4.0 * P.mu / 3.0, P.gm1 * P.kappa) * inv_h * inv_h;
-    ArkViscCoef KV;
-    KV.cn = P.mu * inv_h; KV.ct = 0.25 * P.mu * inv_h; KV.c43 = (4.0 / 3.0) * P.mu * inv_h;
-    KV.c23t = (2.0 / 3.0) * 0.25 * P.mu * inv_h; KV.kh = P.kappa * inv_h;
+    const ArkStepConst K = ark_step_const(P, dt_value, dt_dev);
+    const double lam = K.lam;
 
     const long long colbase = (long long)(li + ARK_XOFF) + (long long)P.px * (long long)(lj + ARK_NG);
     const long long pstride = (long long)P.px * P.py;
@@ -141,171 +185,166 @@ ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict
     double* __restrict__ Ocol = Uout + colbase + pstride * (long long)P.offz;
     const long long fs = P.fstride;
 
-    auto loadU = [&](int k, double* u5) {
+    auto prefetch = [&](int k, int slot) {            // U^n(k) of the own column -> UR[slot]
         const double* __restrict__ c = Ucol + pstride * (long long)k;
-        u5[0] = c[0];
-        u5[1] = c[fs];
-        u5[2] = c[2 * fs];
-        u5[3] = NDIM == 3 ? c[3 * fs] : 0.0;
-        u5[4] = c[FE * fs];
+        double* d = UR + slot * 5 * NCOL + tc;
+        ark_cp_async8(d, c);
+        ark_cp_async8(d + NCOL, c + fs);
+        ark_cp_async8(d + 2 * NCOL, c + 2 * fs);
+        ark_cp_async8(d + 3 * NCOL, c + 3 * fs);
+        ark_cp_async8(d + 4 * NCOL, c + 4 * fs);
     };
-    auto pb = [&](int slot, int f, int col) -> double& { return PB[(slot * ARK_NPRIM + f) * NCOL + col]; };
+    auto primsOf = [&](int slot) {
+        const double* u = UR + slot * 5 * NCOL + tc;
+        return ark_prim_fast(P, u[0], u[NCOL], u[2 * NCOL], u[3 * NCOL], u[4 * NCOL]);
+    };
     auto storePrim = [&](int slot, const ArkPrim& w) {
-        pb(slot, 0, tc) = w.rho; pb(slot, 1, tc) = w.u; pb(slot, 2, tc) = w.v;
-        if (NDIM == 3) pb(slot, 3, tc) = w.w;
-        pb(slot, 4, tc) = w.p; pb(slot, 5, tc) = w.rc; pb(slot, 6, tc) = w.irc;
-        if (VISC) pb(slot, 7, tc) = w.T;
+        double* p = PB + slot * NP * NCOL + tc;
+        p[0] = w.rho; p[NCOL] = w.u; p[2 * NCOL] = w.v; p[3 * NCOL] = w.w;
+        p[4 * NCOL] = w.p; p[5 * NCOL] = w.rc; p[6 * NCOL] = w.irc;
+        if (VISC) p[7 * NCOL] = w.T;
     };
 
+    // ring slots: UR by plane - (k0-2) mod 3; PB likewise (2 slots when the q-1 plane is not needed)
+    int uq = 1, un = 2, unn = 0;                   // planes q, q+1, q+2 at q = k0-1
+    int pm = 0, pc = VISC ? 1 : 0, pn = VISC ? 2 : 1;
+    int tq = 0;                                    // TB slot of plane q
+
+    // ---- prologue: planes k0-2, k0-1 (and k0 in flight)
+    prefetch(k0 - 2, 0); ark_cp_async_commit();
+    prefetch(k0 - 1, 1); ark_cp_async_commit();
+    prefetch(k0, 2);     ark_cp_async_commit();
+    ark_cp_async_wait<1>();
+    ArkFace zlo;
+    {
+        const ArkPrim wm = primsOf(0);
+        const ArkPrim wc0 = primsOf(1);
+        if (VISC) {
+            double* p = PB + pm * NP * NCOL + tc;
+            p[NCOL] = wm.u; p[2 * NCOL] = wm.v; p[3 * NCOL] = wm.w; p[7 * NCOL] = wm.T;
+        }
+        storePrim(pc, wc0);
+        zlo = ark_face(K.th, K.ghz, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
+    }
+    double acc[5] = {0, 0, 0, 0, 0};            // U^{n+1}(q-1) minus its high-z flux
+    double gpz[4] = {0, 0, 0, 0};               // dxw,dxu,dyw,dyv of the own column at q-1 (viscous z face)
     ark_u64 rate_max = 0;
 
-    // ---------------------------------------------------------------------------------------------
-    // register pipeline along z
-    // ---------------------------------------------------------------------------------------------
-    double Ucur[5], Unext[5];          // U^n(q), U^n(q+1)
-    ArkPrim wc, wn;                    // primitives of own column at q, q+1
-    double wmu = 0, wmv = 0, wmw = 0, wmT = 0;  // u,v,w,T of own column at q-1 (viscous z stencil)
-    ArkFace zlo = {0, 0, 0}, zhi = {0, 0, 0};   // acoustic z faces (q-1|q), (q|q+1)
-    double Utprev[5] = {0, 0, 0, 0, 0};         // U~(q-1) of own column
-    double acc[5] = {0, 0, 0, 0, 0};            // U^{n+1}(q-1) minus its high-z flux
-    double gpz[4] = {0, 0, 0, 0};               // dxw,dxu,dyw,dyv of own column at q-1 (viscous z face)
-    int sc = 0, sn = 1;                // PB slots of planes q, q+1
+    for (int q = k0 - 1; q <= k1; ++q) {
+        // ---------------- S1: prefetch plane q+2, primitives of plane q+1
+        if (q + 2 <= k1 + 1) prefetch(q + 2, unn);
+        ark_cp_async_commit();
+        ark_cp_async_wait<1>();                                   // plane q+1 of the own column has landed
+        const ArkPrim wn = primsOf(un);
+        storePrim(pn, wn);
+        __syncthreads();                                          // (A) prims visible
 
-    if (NDIM == 3) {
-        // prologue: planes k0-2 and k0-1
-        double Ua[5];
-        loadU(k0 - 2, Ua);
-        const ArkPrim wm = ark_prim(P, Ua[0], Ua[1], Ua[2], Ua[3], Ua[4]);
-        loadU(k0 - 1, Ucur);
-        wc = ark_prim(P, Ucur[0], Ucur[1], Ucur[2], Ucur[3], Ucur[4]);
-        storePrim(sc, wc);
-        zlo = ark_face(th, ghz, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc.rho, wc.w, wc.p, wc.rc, wc.irc);
-        wmu = wm.u; wmv = wm.v; wmw = wm.w; wmT = wm.T;
-        loadU(k0, Unext);
-    } else {
-        loadU(0, Unext);
-        wc = ark_prim(P, Unext[0], Unext[1], Unext[2], Unext[3], Unext[4]);
-    }
-
-    const int qbeg = NDIM == 3 ? k0 - 1 : 0, qend = NDIM == 3 ? k1 : 0;
-    for (int q = qbeg; q <= qend; ++q) {
-        // ---------------- S1: primitives of plane q+1 (3D) / plane 0 (2D)
-        double Upre[5] = {0, 0, 0, 0, 0};
-        if (NDIM == 3) {
-            if (q + 2 <= k1 + 1) loadU(q + 2, Upre);           // prefetch, consumed next iteration
-            wn = ark_prim(P, Unext[0], Unext[1], Unext[2], Unext[3], Unext[4]);
-            storePrim(sn, wn);
-        } else {
-            for (int f = 0; f < 5; ++f) Ucur[f] = Unext[f];
-            wn = wc;
-            storePrim(sc, wc);
-        }
-        __syncthreads();                                       // (A) prims visible
-
-        const bool do_update = NDIM == 2 || (q >= k0 && q < k1);   // plane q is an output plane of this chunk
-        // ---------------- S2: acoustic faces of plane q
-        ArkFace fx = {0, 0, 0}, fy = {0, 0, 0};
-        if (inFx) {
-            const int n = tc - 1;
-            fx = ark_face(th, ghx, pb(sc, 0, n), pb(sc, 1, n), pb(sc, 4, n), pb(sc, 5, n), pb(sc, 6, n),
-                          wc.rho, wc.u, wc.p, wc.rc, wc.irc);
-            FB[0 * NCOL + tc] = fx.us; FB[1 * NCOL + tc] = fx.pi;
-            if (gx_on) FB[4 * NCOL + tc] = fx.S;
-        }
-        if (inFy) {
-            const int n = tc - RX;
-            fy = ark_face(th, ghy, pb(sc, 0, n), pb(sc, 2, n), pb(sc, 4, n), pb(sc, 5, n), pb(sc, 6, n),
-                          wc.rho, wc.v, wc.p, wc.rc, wc.irc);
-            FB[2 * NCOL + tc] = fy.us; FB[3 * NCOL + tc] = fy.pi;
-            if (gy_on) FB[5 * NCOL + tc] = fy.S;
-        }
-        if (NDIM == 3 && inA)
-            zhi = ark_face(th, ghz, wc.rho, wc.w, wc.p, wc.rc, wc.irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
-
-        // centred velocity differences of plane q (un-normalised: q(+1) - q(-1)), tile + 1 ring
+        const bool do_update = q >= k0 && q < k1;                 // plane q is an output plane of this chunk
+        // ---------------- S2: acoustic faces of plane q, centred velocity differences
+        const double* pq = PB + pc * NP * NCOL + tc;
+        double rho = 0, u = 0, v = 0, w = 0, p = 0, rc = 0, irc = 0;
+        ArkFace fx = {0, 0, 0}, fy = {0, 0, 0}, zhi = {0, 0, 0};
         double dxu = 0, dxv = 0, dxw = 0, dyu = 0, dyv = 0, dyw = 0, dzu = 0, dzv = 0, dzw = 0;
-        if (VISC && inA) {
-            dxu = pb(sc, 1, tc + 1) - pb(sc, 1, tc - 1);
-            dxv = pb(sc, 2, tc + 1) - pb(sc, 2, tc - 1);
-            dyu = pb(sc, 1, tc + RX) - pb(sc, 1, tc - RX);
-            dyv = pb(sc, 2, tc + RX) - pb(sc, 2, tc - RX);
-            if (NDIM == 3) {
-                dxw = pb(sc, 3, tc + 1) - pb(sc, 3, tc - 1);
-                dyw = pb(sc, 3, tc + RX) - pb(sc, 3, tc - RX);
-                dzu = wn.u - wmu; dzv = wn.v - wmv; dzw = wn.w - wmw;
+        if (rowF) {
+            rho = pq[0]; u = pq[NCOL]; v = pq[2 * NCOL]; w = pq[3 * NCOL]; p = pq[4 * NCOL]; rc = pq[5 * NCOL]; irc = pq[6 * NCOL];
+            {
+                const double* n = pq - RX;
+                fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
+                FB[2 * NCOL + tc] = fy.us; FB[3 * NCOL + tc] = fy.pi;
+                if (K.gy_on) FB[5 * NCOL + tc] = fy.S;
             }
-            GB[0 * NCOL + tc] = dyu; GB[1 * NCOL + tc] = dyv;
-            GB[4 * NCOL + tc] = dxv; GB[5 * NCOL + tc] = dxu;
-            if (NDIM == 3) { GB[2 * NCOL + tc] = dzu; GB[3 * NCOL + tc] = dzw; GB[6 * NCOL + tc] = dzv; }
+            if (rowA) {
+                const double* n = pq - 1;
+                fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
+                FB[0 * NCOL + tc] = fx.us; FB[1 * NCOL + tc] = fx.pi;
+                if (K.gx_on) FB[4 * NCOL + tc] = fx.S;
+                zhi = ark_face(K.th, K.ghz, rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
+                if (VISC) {
+                    // un-normalised centred differences q(+1) - q(-1)
+                    dxu = pq[NCOL + 1] - pq[NCOL - 1];
+                    dxv = pq[2 * NCOL + 1] - pq[2 * NCOL - 1];
+                    dxw = pq[3 * NCOL + 1] - pq[3 * NCOL - 1];
+                    dyu = pq[NCOL + RX] - pq[NCOL - RX];
+                    dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
+                    dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
+                    const double* pmn = PB + pm * NP * NCOL + tc;
+                    dzu = wn.u - pmn[NCOL]; dzv = wn.v - pmn[2 * NCOL]; dzw = wn.w - pmn[3 * NCOL];
+                    GB[0 * NCOL + tc] = dyu; GB[1 * NCOL + tc] = dyv; GB[2 * NCOL + tc] = dzu; GB[3 * NCOL + tc] = dzw;
+                    GB[4 * NCOL + tc] = dxv; GB[5 * NCOL + tc] = dxu; GB[6 * NCOL + tc] = dzv;
+                }
+            }
         }
-        __syncthreads();                                       // (B) faces and differences visible
+        __syncthreads();                                          // (B) faces and differences visible
 
         // ---------------- S3: acoustic update U~(q), PAPER.md:158-160 (+ reading A3 for the energy)
-        double Ut[5] = {0, 0, 0, 0, 0};
+        double Uc[5] = {0, 0, 0, 0, 0}, Ut[5] = {0, 0, 0, 0, 0};
         double usxh = 0, pixh = 0, usyh = 0, piyh = 0, Six = 0, Siy = 0, Siz = 0;
-        if (inA) {
+        ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
+        if (rowA) {
+            const double* uc = UR + uq * 5 * NCOL + tc;
+            Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
             usxh = FB[0 * NCOL + tc + 1]; pixh = FB[1 * NCOL + tc + 1];
             usyh = FB[2 * NCOL + tc + RX]; piyh = FB[3 * NCOL + tc + RX];
-            if (gx_on) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
-            if (gy_on) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
-            double sdu = (usxh - fx.us) + (usyh - fy.us);
-            double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us);
-            if (NDIM == 3) {
-                sdu += zhi.us - zlo.us;
-                sdpu += zhi.pi * zhi.us - zlo.pi * zlo.us;
-                Siz = 0.5 * (zhi.S + zlo.S);
-            }
-            const double iLt = 1.0 / (1.0 + lam * sdu);
-            Ut[0] = Ucur[0] * iLt;
-            Ut[1] = (Ucur[1] - lam * (pixh - fx.pi) + lam * Six) * iLt;
-            Ut[2] = (Ucur[2] - lam * (piyh - fy.pi) + lam * Siy) * iLt;
-            if (NDIM == 3) Ut[3] = (Ucur[3] - lam * (zhi.pi - zlo.pi) + lam * Siz) * iLt;
-            Ut[4] = (Ucur[4] - lam * sdpu) * iLt;
-            TB[0 * NCOL + tc] = Ut[0]; TB[1 * NCOL + tc] = Ut[1]; TB[2 * NCOL + tc] = Ut[2];
-            if (NDIM == 3) TB[3 * NCOL + tc] = Ut[3];
-            TB[4 * NCOL + tc] = Ut[4];
+            if (K.gx_on) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
+            if (K.gy_on) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
+            Siz = 0.5 * (zhi.S + zlo.S);
+            const double sdu = (usxh - fx.us) + (usyh - fy.us) + (zhi.us - zlo.us);
+            const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us) + (zhi.pi * zhi.us - zlo.pi * zlo.us);
+            const double iLt = ark_rcp(1.0 + lam * sdu);
+            Ut[0] = Uc[0] * iLt;
+            Ut[1] = (Uc[1] - lam * (pixh - fx.pi) + lam * Six) * iLt;
+            Ut[2] = (Uc[2] - lam * (piyh - fy.pi) + lam * Siy) * iLt;
+            Ut[3] = (Uc[3] - lam * (zhi.pi - zlo.pi) + lam * Siz) * iLt;
+            Ut[4] = (Uc[4] - lam * sdpu) * iLt;
+            double* tb = TB + tq * 5 * NCOL + tc;
+            tb[0] = Ut[0]; tb[NCOL] = Ut[1]; tb[2 * NCOL] = Ut[2]; tb[3 * NCOL] = Ut[3]; tb[4 * NCOL] = Ut[4];
         }
-
         // viscous / heat fluxes through the low x, low y faces of plane q and the z face (q-1 | q)
-        ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
         if (VISC) {
-            if (do_update && inVx) {   // face (ci-1 | ci), normal x, transverse a = y, b = z
-                const int L = tc - 1;
-                const double uL = pb(sc, 1, L), vL = pb(sc, 2, L), wL = NDIM == 3 ? pb(sc, 3, L) : 0.0, TL = pb(sc, 7, L);
-                const double tra_n = GB[0 * NCOL + L] + dyu, tra_a = GB[1 * NCOL + L] + dyv;
-                const double trb_n = NDIM == 3 ? GB[2 * NCOL + L] + dzu : 0.0, trb_b = NDIM == 3 ? GB[3 * NCOL + L] + dzw : 0.0;
-                vx = ark_visc_face(KV, wc.u - uL, wc.v - vL, wc.w - wL, tra_n, tra_a, trb_n, trb_b,
-                                   uL + wc.u, vL + wc.v, wL + wc.w, wc.T - TL);
-                VB[0 * NCOL + tc] = vx.t0; VB[1 * NCOL + tc] = vx.t1; VB[3 * NCOL + tc] = vx.fe;
-                if (NDIM == 3) VB[2 * NCOL + tc] = vx.t2;
+            if (rowVy) {
+                const double Tc = pq[7 * NCOL];
+                if (do_update) {
+                    if (rowU) {    // face (ci-1 | ci), normal x, transverse a = y, b = z
+                        const double* L = pq - 1;
+                        const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
+                        const int l = tc - 1;
+                        vx = ark_visc_face(K.KV, u - uL, v - vL, w - wL, GB[0 * NCOL + l] + dyu, GB[1 * NCOL + l] + dyv,
+                                           GB[2 * NCOL + l] + dzu, GB[3 * NCOL + l] + dzw, uL + u, vL + v, wL + w, Tc - TL);
+                        VB[0 * NCOL + tc] = vx.t0; VB[1 * NCOL + tc] = vx.t1; VB[2 * NCOL + tc] = vx.t2; VB[3 * NCOL + tc] = vx.fe;
+                    }
+                    {              // face (cj-1 | cj), normal y, transverse a = x, b = z
+                        const double* L = pq - RX;
+                        const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
+                        const int l = tc - RX;
+                        vy = ark_visc_face(K.KV, v - vL, u - uL, w - wL, GB[4 * NCOL + l] + dxv, GB[5 * NCOL + l] + dxu,
+                                           GB[6 * NCOL + l] + dzv, GB[3 * NCOL + l] + dzw, vL + v, uL + u, wL + w, Tc - TL);
+                        // stored as (tau_yx, tau_yy, tau_yz, fe): component order x,y,z
+                        VB[4 * NCOL + tc] = vy.t1; VB[5 * NCOL + tc] = vy.t0; VB[6 * NCOL + tc] = vy.t2; VB[7 * NCOL + tc] = vy.fe;
+                    }
+                }
+                if (rowU && q >= k0) {   // face (q-1 | q), normal z, transverse a = x, b = y
+                    const double* pmn = PB + pm * NP * NCOL + tc;
+                    const double um = pmn[NCOL], vm = pmn[2 * NCOL], wm = pmn[3 * NCOL], Tm = pmn[7 * NCOL];
+                    vz = ark_visc_face(K.KV, w - wm, u - um, v - vm, gpz[0] + dxw, gpz[1] + dxu, gpz[2] + dyw, gpz[3] + dyv,
+                                       wm + w, um + u, vm + v, Tc - Tm);
+                }
             }
-            if (do_update && inVy) {   // face (cj-1 | cj), normal y, transverse a = x, b = z
-                const int L = tc - RX;
-                const double uL = pb(sc, 1, L), vL = pb(sc, 2, L), wL = NDIM == 3 ? pb(sc, 3, L) : 0.0, TL = pb(sc, 7, L);
-                const double tra_n = GB[4 * NCOL + L] + dxv, tra_a = GB[5 * NCOL + L] + dxu;
-                const double trb_n = NDIM == 3 ? GB[6 * NCOL + L] + dzv : 0.0, trb_b = NDIM == 3 ? GB[3 * NCOL + L] + dzw : 0.0;
-                vy = ark_visc_face(KV, wc.v - vL, wc.u - uL, wc.w - wL, tra_n, tra_a, trb_n, trb_b,
-                                   vL + wc.v, uL + wc.u, wL + wc.w, wc.T - TL);
-                // stored as (tau_yx, tau_yy, tau_yz, fe): component order x,y,z
-                VB[4 * NCOL + tc] = vy.t1; VB[5 * NCOL + tc] = vy.t0; VB[7 * NCOL + tc] = vy.fe;
-                if (NDIM == 3) VB[6 * NCOL + tc] = vy.t2;
-            }
-            if (NDIM == 3) {
-                if (inU && q >= k0)    // face (q-1 | q), normal z, transverse a = x, b = y
-                    vz = ark_visc_face(KV, wc.w - wmw, wc.u - wmu, wc.v - wmv, gpz[0] + dxw, gpz[1] + dxu, gpz[2] + dyw, gpz[3] + dyv,
-                                       wmw + wc.w, wmu + wc.u, wmv + wc.v, wc.T - wmT);
-                gpz[0] = dxw; gpz[1] = dxu; gpz[2] = dyw; gpz[3] = dyv;
-            }
+            gpz[0] = dxw; gpz[1] = dxu; gpz[2] = dyw; gpz[3] = dyv;
         }
-        __syncthreads();                                       // (C) U~(q) and viscous fluxes visible
+        __syncthreads();                                          // (C) U~(q) and viscous fluxes visible
 
         // ---------------- S4: transport + update
-        if (inU) {
+        if (rowU) {
+            const double* Tq = TB + tq * 5 * NCOL;
             double Gz[5] = {0, 0, 0, 0, 0};       // full flux through the z face (q-1|q)
             double mzf = 0.0;
-            if (NDIM == 3 && q >= k0) {
-                const bool up = zlo.us >= 0.0;                  // PAPER.md:174, reading A10
-                for (int f = 0; f < 5; ++f) Gz[f] = (up ? Utprev[f] : Ut[f]) * zlo.us;
+            if (q >= k0) {
+                const double* Tp = TB + (tq ^ 1) * 5 * NCOL + tc;     // U~(q-1), own column
+                if (ark_nonneg(zlo.us)) {                             // PAPER.md:174, reading A10
+                    for (int f = 0; f < 5; ++f) Gz[f] = Tp[f * NCOL] * zlo.us;
+                } else {
+                    for (int f = 0; f < 5; ++f) Gz[f] = Ut[f] * zlo.us;
+                }
                 mzf = Gz[0];
                 Gz[3] += zlo.pi;
                 Gz[4] += zlo.pi * zlo.us;
@@ -314,79 +353,48 @@ ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict
                     // complete and store U^{n+1}(q-1):  acc - lam * G_z(high) + gravity work of the high face
                     double out[5];
                     for (int f = 0; f < 5; ++f) out[f] = acc[f] - lam * Gz[f];
-                    if (ghz != 0.0) out[4] += dt * P.g[2] * (mzf < 0.0 ? mzf : 0.0);
-                    double* __restrict__ c = Ocol + pstride * (long long)(q - 1);
-                    c[0] = out[0];
-                    c[fs] = out[1];
-                    c[2 * fs] = out[2];
-                    c[3 * fs] = out[3];
-                    c[FE * fs] = out[4];
-                    if (rate_scratch) rate_max = ark_umax(rate_max, ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], inv_h, dcoef));
+                    if (K.gz_on) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
+                    if (inU) {
+                        double* __restrict__ c = Ocol + pstride * (long long)(q - 1);
+                        c[0] = out[0];
+                        c[fs] = out[1];
+                        c[2 * fs] = out[2];
+                        c[3 * fs] = out[3];
+                        c[4 * fs] = out[4];
+                        if (rate_scratch) rate_max = ark_umax(rate_max, ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], K.inv_h, K.dcoef));
+                    }
                 }
             }
             if (do_update) {
-                // in-plane faces of plane q: F = U~_up u* + (0, Pi* e_d, Pi* u*) - D ; dG = sum_d (F_d+ - F_d-)
+                // in-plane faces of plane q: dG = sum_d (F_d+ - F_d-)
                 double dG[5];
                 double work = 0.0;
-                {   // x axis
-                    const double usl = fx.us, ush = usxh;
-                    const int nl = usl >= 0.0 ? tc - 1 : tc, nh = ush >= 0.0 ? tc : tc + 1;
-                    const double ml = TB[nl] * usl, mh = TB[nh] * ush;
-                    dG[0] = mh - ml;
-                    dG[1] = (TB[NCOL + nh] * ush + pixh) - (TB[NCOL + nl] * usl + fx.pi);
-                    dG[2] = TB[2 * NCOL + nh] * ush - TB[2 * NCOL + nl] * usl;
-                    dG[3] = NDIM == 3 ? TB[3 * NCOL + nh] * ush - TB[3 * NCOL + nl] * usl : 0.0;
-                    dG[4] = (TB[4 * NCOL + nh] + pixh) * ush - (TB[4 * NCOL + nl] + fx.pi) * usl;
-                    if (gx_on) work += P.g[0] * ((ml > 0.0 ? ml : 0.0) + (mh < 0.0 ? mh : 0.0));
-                }
-                {   // y axis
-                    const double usl = fy.us, ush = usyh;
-                    const int nl = usl >= 0.0 ? tc - RX : tc, nh = ush >= 0.0 ? tc : tc + RX;
-                    const double ml = TB[nl] * usl, mh = TB[nh] * ush;
-                    dG[0] += mh - ml;
-                    dG[1] += TB[NCOL + nh] * ush - TB[NCOL + nl] * usl;
-                    dG[2] += (TB[2 * NCOL + nh] * ush + piyh) - (TB[2 * NCOL + nl] * usl + fy.pi);
-                    if (NDIM == 3) dG[3] += TB[3 * NCOL + nh] * ush - TB[3 * NCOL + nl] * usl;
-                    dG[4] += (TB[4 * NCOL + nh] + piyh) * ush - (TB[4 * NCOL + nl] + fy.pi) * usl;
-                    if (gy_on) work += P.g[1] * ((ml > 0.0 ? ml : 0.0) + (mh < 0.0 ? mh : 0.0));
-                }
+                ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
+                ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
                 if (VISC) {
                     dG[1] -= (VB[0 * NCOL + tc + 1] - vx.t0) + (VB[4 * NCOL + tc + RX] - vy.t1);
                     dG[2] -= (VB[1 * NCOL + tc + 1] - vx.t1) + (VB[5 * NCOL + tc + RX] - vy.t0);
-                    if (NDIM == 3) dG[3] -= (VB[2 * NCOL + tc + 1] - vx.t2) + (VB[6 * NCOL + tc + RX] - vy.t2);
+                    dG[3] -= (VB[2 * NCOL + tc + 1] - vx.t2) + (VB[6 * NCOL + tc + RX] - vy.t2);
                     dG[4] -= (VB[3 * NCOL + tc + 1] - vx.fe) + (VB[7 * NCOL + tc + RX] - vy.fe);
                 }
-                double nw[5];
-                nw[0] = Ucur[0] - lam * dG[0];
-                nw[1] = Ucur[1] - lam * dG[1] + lam * Six;
-                nw[2] = Ucur[2] - lam * dG[2] + lam * Siy;
-                nw[3] = Ucur[3] - lam * dG[3];
-                nw[4] = Ucur[4] - lam * dG[4] + dt * work;
-                if (NDIM == 3) {
-                    // low z face enters with +lam*G_z and the gravity work dt g_z max(m,0); the source lam*S_i
-                    for (int f = 0; f < 5; ++f) acc[f] = nw[f] + lam * Gz[f];
-                    if (ghz != 0.0) {
-                        acc[3] += lam * Siz;
-                        acc[4] += dt * P.g[2] * (mzf > 0.0 ? mzf : 0.0);
-                    }
-                } else {
-                    double* __restrict__ c = Ocol;
-                    c[0] = nw[0];
-                    c[fs] = nw[1];
-                    c[2 * fs] = nw[2];
-                    c[FE * fs] = nw[4];
-                    if (rate_scratch) rate_max = ark_umax(rate_max, ark_rate_epilogue(P, 2, nw[0], nw[1], nw[2], 0.0, nw[4], inv_h, dcoef));
+                // low z face enters with +lam*G_z and the gravity work dt g_z max(m,0); the source lam*S_i
+                acc[0] = (Uc[0] - lam * dG[0]) + lam * Gz[0];
+                acc[1] = (Uc[1] - lam * dG[1] + lam * Six) + lam * Gz[1];
+                acc[2] = (Uc[2] - lam * dG[2] + lam * Siy) + lam * Gz[2];
+                acc[3] = (Uc[3] - lam * dG[3]) + lam * Gz[3];
+                acc[4] = (Uc[4] - lam * dG[4] + K.dt * work) + lam * Gz[4];
+                if (K.gz_on) {
+                    acc[3] += lam * Siz;
+                    acc[4] += K.dt * P.g[2] * ark_pos_part(mzf);
                 }
             }
         }
-        if (NDIM == 3) {
-            // rotate the z pipeline
-            for (int f = 0; f < 5; ++f) { Utprev[f] = Ut[f]; Ucur[f] = Unext[f]; Unext[f] = Upre[f]; }
-            if (VISC) { wmu = wc.u; wmv = wc.v; wmw = wc.w; wmT = wc.T; }
-            wc = wn;
-            zlo = zhi;
-            sc ^= 1; sn ^= 1;
-        }
+        // rotate the rings
+        zlo = zhi;
+        { const int s = uq; uq = un; un = unn; unn = s; }
+        if (VISC) { const int s = pm; pm = pc; pc = pn; pn = s; }
+        else      { const int s = pc; pc = pn; pn = s; }
+        tq ^= 1;
     }
 
     if (rate_scratch) {
@@ -407,4 +415,160 @@ ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict
 #endif
         if (t == 0) rate_scratch[blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z)] = ark_rate_from_bits(m);
     }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// 2D body: one plane, same phases, direct loads
+// ------------------------------------------------------------------------------------------------------------
+template <bool VISC, int TX, int TY>
+ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
+                        const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, double* smem) {
+    using C = ArkStepCfg<2, VISC, TX, TY>;
+    constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP;
+    double* PB = smem;                                // [NP][NCOL]
+    double* FB = PB + NP * NCOL;                      // [6][NCOL]
+    double* TB = FB + 6 * NCOL;                       // [5][NCOL] (component 3 unused)
+    double* GB = TB + 5 * NCOL;                       // [7][NCOL] (VISC)
+    double* VB = GB + (VISC ? 7 : 0) * NCOL;          // [8][NCOL] (VISC)
+    ark_u64* red = (ark_u64*)(VB + (VISC ? 8 : 0) * NCOL);
+
+    const int t = threadIdx.x;
+    const int tc = t < NCOL ? t : NCOL - 1;
+    const int ci = tc % RX, cj = tc / RX;
+    const int gi = blockIdx.x * TX - 2 + ci, gj = blockIdx.y * TY - 2 + cj;
+    const int li = gi < P.nx + 2 ? gi : P.nx + 1;
+    const int lj = gj < P.ny + 2 ? gj : P.ny + 1;
+    const bool rowF = cj >= 1;
+    const bool rowA = cj >= 1 && cj <= RY - 2;
+    const bool rowU = cj >= 2 && cj <= RY - 3;
+    const bool rowVy = cj >= 2 && cj <= RY - 2;
+    const bool inU = t < NCOL && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;
+
+    const ArkStepConst K = ark_step_const(P, dt_value, dt_dev);
+    const double lam = K.lam;
+    const long long colbase = (long long)(li + ARK_XOFF) + (long long)P.px * (long long)(lj + ARK_NG);
+    const long long fs = P.fstride;
+
+    // S1
+    double Uc[5];
+    Uc[0] = Uin[colbase]; Uc[1] = Uin[colbase + fs]; Uc[2] = Uin[colbase + 2 * fs]; Uc[3] = 0.0; Uc[4] = Uin[colbase + 3 * fs];
+    const ArkPrim wc = ark_prim_fast(P, Uc[0], Uc[1], Uc[2], 0.0, Uc[4]);
+    {
+        double* p = PB + tc;
+        p[0] = wc.rho; p[NCOL] = wc.u; p[2 * NCOL] = wc.v; p[4 * NCOL] = wc.p; p[5 * NCOL] = wc.rc; p[6 * NCOL] = wc.irc;
+        if (VISC) p[7 * NCOL] = wc.T;
+    }
+    __syncthreads();
+    // S2
+    const double* pq = PB + tc;
+    ArkFace fx = {0, 0, 0}, fy = {0, 0, 0};
+    double dxu = 0, dxv = 0, dyu = 0, dyv = 0;
+    if (rowF) {
+        {
+            const double* n = pq - RX;
+            fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.v, wc.p, wc.rc, wc.irc);
+            FB[2 * NCOL + tc] = fy.us; FB[3 * NCOL + tc] = fy.pi;
+            if (K.gy_on) FB[5 * NCOL + tc] = fy.S;
+        }
+        if (rowA) {
+            const double* n = pq - 1;
+            fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.u, wc.p, wc.rc, wc.irc);
+            FB[0 * NCOL + tc] = fx.us; FB[1 * NCOL + tc] = fx.pi;
+            if (K.gx_on) FB[4 * NCOL + tc] = fx.S;
+            if (VISC) {
+                dxu = pq[NCOL + 1] - pq[NCOL - 1];
+                dxv = pq[2 * NCOL + 1] - pq[2 * NCOL - 1];
+                dyu = pq[NCOL + RX] - pq[NCOL - RX];
+                dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
+                GB[0 * NCOL + tc] = dyu; GB[1 * NCOL + tc] = dyv; GB[4 * NCOL + tc] = dxv; GB[5 * NCOL + tc] = dxu;
+            }
+        }
+    }
+    __syncthreads();
+    // S3
+    double usxh = 0, pixh = 0, usyh = 0, piyh = 0, Six = 0, Siy = 0;
+    ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0};
+    if (rowA) {
+        usxh = FB[0 * NCOL + tc + 1]; pixh = FB[1 * NCOL + tc + 1];
+        usyh = FB[2 * NCOL + tc + RX]; piyh = FB[3 * NCOL + tc + RX];
+        if (K.gx_on) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
+        if (K.gy_on) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
+        const double sdu = (usxh - fx.us) + (usyh - fy.us);
+        const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us);
+        const double iLt = ark_rcp(1.0 + lam * sdu);
+        double* tb = TB + tc;
+        tb[0] = Uc[0] * iLt;
+        tb[NCOL] = (Uc[1] - lam * (pixh - fx.pi) + lam * Six) * iLt;
+        tb[2 * NCOL] = (Uc[2] - lam * (piyh - fy.pi) + lam * Siy) * iLt;
+        tb[4 * NCOL] = (Uc[4] - lam * sdpu) * iLt;
+    }
+    if (VISC && rowVy) {
+        if (rowU) {
+            const double* L = pq - 1;
+            const double uL = L[NCOL], vL = L[2 * NCOL], TL = L[7 * NCOL];
+            const int l = tc - 1;
+            vx = ark_visc_face(K.KV, wc.u - uL, wc.v - vL, 0.0, GB[0 * NCOL + l] + dyu, GB[1 * NCOL + l] + dyv, 0.0, 0.0,
+                               uL + wc.u, vL + wc.v, 0.0, wc.T - TL);
+            VB[0 * NCOL + tc] = vx.t0; VB[1 * NCOL + tc] = vx.t1; VB[3 * NCOL + tc] = vx.fe;
+        }
+        {
+            const double* L = pq - RX;
+            const double uL = L[NCOL], vL = L[2 * NCOL], TL = L[7 * NCOL];
+            const int l = tc - RX;
+            vy = ark_visc_face(K.KV, wc.v - vL, wc.u - uL, 0.0, GB[4 * NCOL + l] + dxv, GB[5 * NCOL + l] + dxu, 0.0, 0.0,
+                               vL + wc.v, uL + wc.u, 0.0, wc.T - TL);
+            VB[4 * NCOL + tc] = vy.t1; VB[5 * NCOL + tc] = vy.t0; VB[7 * NCOL + tc] = vy.fe;
+        }
+    }
+    __syncthreads();
+    // S4
+    ark_u64 rate_max = 0;
+    if (rowU) {
+        double dG[5];
+        double work = 0.0;
+        ark_transport_axis<2, 1>(TB, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
+        ark_transport_axis<2, 2>(TB, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
+        if (VISC) {
+            dG[1] -= (VB[0 * NCOL + tc + 1] - vx.t0) + (VB[4 * NCOL + tc + RX] - vy.t1);
+            dG[2] -= (VB[1 * NCOL + tc + 1] - vx.t1) + (VB[5 * NCOL + tc + RX] - vy.t0);
+            dG[4] -= (VB[3 * NCOL + tc + 1] - vx.fe) + (VB[7 * NCOL + tc + RX] - vy.fe);
+        }
+        const double n0 = Uc[0] - lam * dG[0];
+        const double n1 = Uc[1] - lam * dG[1] + lam * Six;
+        const double n2 = Uc[2] - lam * dG[2] + lam * Siy;
+        const double n4 = Uc[4] - lam * dG[4] + K.dt * work;
+        if (inU) {
+            Uout[colbase] = n0; Uout[colbase + fs] = n1; Uout[colbase + 2 * fs] = n2; Uout[colbase + 3 * fs] = n4;
+            if (rate_scratch) rate_max = ark_rate_epilogue(P, 2, n0, n1, n2, 0.0, n4, K.inv_h, K.dcoef);
+        }
+    }
+    if (rate_scratch) {
+        ark_u64 m = rate_max;
+#ifndef ARK_HOST_EMU
+        for (int o = 16; o > 0; o >>= 1) m = ark_umax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        const int lane = t & 31, wid = t >> 5;
+        if (lane == 0) red[wid] = m;
+        __syncthreads();
+        if (wid == 0) {
+            m = lane < (int)(C::NT / 32) ? red[lane] : 0;
+            for (int o = 16; o > 0; o >>= 1) m = ark_umax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        }
+#else
+        m = ark_emu_block_umax(m);
+        (void)red;
+#endif
+        if (t == 0) rate_scratch[blockIdx.x + gridDim.x * blockIdx.y] = ark_rate_from_bits(m);
+    }
+}
+
+template <int NDIM, bool VISC, int TX, int TY>
+ARK_GLOBAL void
+#ifndef ARK_HOST_EMU
+__launch_bounds__(ArkStepCfg<NDIM, VISC, TX, TY>::NT, 1)
+#endif
+ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict__ Uout,
+           double dt_value, const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk) {
+    ARK_DYN_SMEM(smem);
+    if (NDIM == 3) ark_step3d<VISC, TX, TY>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, zchunk, smem);
+    else           ark_step2d<VISC, TX, TY>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, smem);
 }

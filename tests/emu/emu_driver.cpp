@@ -34,7 +34,7 @@ void bc(const ArkParams& P, double* U, long long n) {
 
 template <int NDIM, bool VISC>
 void step(const ArkParams& P, const double* Uin, double* Uout, double dt, double* scratch, int zchunk, emu_dim3 grid) {
-    using C = ArkStepCfg<ETX, ETY>;
+    using C = ArkStepCfg<NDIM, VISC, ETX, ETY>;
     ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch, zchunk); });
 }
 }  // namespace
