@@ -143,263 +143,310 @@ ARK_DEV void ark_transport_axis(const double* __restrict__ T, int cs, int tc, in
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// 3D body
+// 3D body.  The march is specialised by ROW ROLE (a compile-time parameter of the whole plane loop, chosen once
+// per thread and warp-uniform when RX == 32) so that no role test, no predicate and no dummy initialisation is
+// left inside an iteration:
+//   ROLE 0  edge rows 0, RY-1 : primitives, low-y acoustic face
+//   ROLE 1  ring rows 1, RY-2 : + low-x / high-z faces, centred differences, U~, viscous low-y face
+//   ROLE 2  tile rows 2..RY-3 : + viscous x / z faces, transport, update, store, CFL rate
+// and by STEADY (planes k0+1 .. k1-1, where every chunk-boundary condition is known) vs. the generic first and
+// last iterations.  Every role executes the same two barriers per plane.
 // ------------------------------------------------------------------------------------------------------------
+template <bool VISC, int TX, int TY>
+struct ArkMarch {
+    double *UR, *PB, *FB, *TB, *GB, *VB;
+    const double* Ucol;
+    double* Ocol;
+    long long pstride, fs;
+    int tc, k0, k1;
+    bool inU, want_rate;
+    int uq, un, unn, pm, pc, pn, tq;     // ring slots of planes q, q+1, q+2 (UR); q-1, q, q+1 (PB); q (TB)
+    ArkFace zlo;                         // acoustic z face (q-1|q)
+    double acc[5];                       // U^{n+1}(q-1) minus its high-z flux
+    double gpz[4];                       // dxw,dxu,dyw,dyv of the own column at q-1 (viscous z face)
+    ark_u64 rate_max;
+};
+
+template <bool VISC, int TX, int TY>
+ARK_DEV void ark_march_prefetch(const ArkMarch<VISC, TX, TY>& M, int k, int slot) {   // U^n(k), own column -> UR[slot]
+    constexpr int NCOL = ArkStepCfg<3, VISC, TX, TY>::NCOL;
+    const double* __restrict__ c = M.Ucol + M.pstride * (long long)k;
+    double* d = M.UR + slot * 5 * NCOL + M.tc;
+    ark_cp_async8(d, c);
+    ark_cp_async8(d + NCOL, c + M.fs);
+    ark_cp_async8(d + 2 * NCOL, c + 2 * M.fs);
+    ark_cp_async8(d + 3 * NCOL, c + 3 * M.fs);
+    ark_cp_async8(d + 4 * NCOL, c + 4 * M.fs);
+}
+
+template <bool VISC, int TX, int TY>
+ARK_DEV ArkPrim ark_march_prims(const ArkParams& P, const ArkMarch<VISC, TX, TY>& M, int slot) {
+    constexpr int NCOL = ArkStepCfg<3, VISC, TX, TY>::NCOL;
+    const double* u = M.UR + slot * 5 * NCOL + M.tc;
+    return ark_prim_fast(P, u[0], u[NCOL], u[2 * NCOL], u[3 * NCOL], u[4 * NCOL]);
+}
+
+template <bool VISC, int TX, int TY, int ROLE, bool STEADY>
+ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC, TX, TY>& M, const int q) {
+    using C = ArkStepCfg<3, VISC, TX, TY>;
+    constexpr int RX = C::RX, NCOL = C::NCOL, NP = C::NP;
+    const int tc = M.tc;
+    const double lam = K.lam;
+    const bool do_update = STEADY || (q >= M.k0 && q < M.k1);     // plane q is an output plane of this chunk
+    const bool has_zlo = STEADY || q >= M.k0;                     // face (q-1|q) bounds an output plane
+    const bool completes = STEADY || q > M.k0;                    // plane q-1 is completed and stored here
+
+    // ---------------- S1: prefetch plane q+2, primitives of plane q+1 (own column)
+    if (STEADY || q + 2 <= M.k1 + 1) ark_march_prefetch(M, q + 2, M.unn);
+    ark_cp_async_commit();
+    ark_cp_async_wait<1>();                                       // plane q+1 of the own column has landed
+    const ArkPrim wn = ark_march_prims(P, M, M.un);
+    {
+        double* p = M.PB + M.pn * NP * NCOL + tc;
+        p[0] = wn.rho; p[NCOL] = wn.u; p[2 * NCOL] = wn.v; p[3 * NCOL] = wn.w;
+        p[4 * NCOL] = wn.p; p[5 * NCOL] = wn.rc; p[6 * NCOL] = wn.irc;
+        if (VISC) p[7 * NCOL] = wn.T;
+    }
+    // (no barrier: S2 reads the neighbours' primitives of plane q, written one iteration ago)
+
+    // ---------------- S2: acoustic faces of plane q, centred velocity differences
+    const double* pq = M.PB + M.pc * NP * NCOL + tc;
+    const double rho = pq[0], u = pq[NCOL], v = pq[2 * NCOL], w = pq[3 * NCOL], p = pq[4 * NCOL], rc = pq[5 * NCOL], irc = pq[6 * NCOL];
+    ArkFace fy;
+    {
+        const double* n = pq - RX;
+        fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
+        M.FB[2 * NCOL + tc] = fy.us; M.FB[3 * NCOL + tc] = fy.pi;
+        if (K.gy_on) M.FB[5 * NCOL + tc] = fy.S;
+    }
+    ArkFace fx = fy, zhi = fy;                                    // (overwritten below for ROLE >= 1)
+    double dxu = 0, dxv = 0, dxw = 0, dyu = 0, dyv = 0, dyw = 0, dzu = 0, dzv = 0, dzw = 0;
+    if (ROLE >= 1) {
+        const double* n = pq - 1;
+        fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
+        M.FB[0 * NCOL + tc] = fx.us; M.FB[1 * NCOL + tc] = fx.pi;
+        if (K.gx_on) M.FB[4 * NCOL + tc] = fx.S;
+        zhi = ark_face(K.th, K.ghz, rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
+        if (VISC) {
+            // un-normalised centred differences q(+1) - q(-1)
+            dxu = pq[NCOL + 1] - pq[NCOL - 1];
+            dxv = pq[2 * NCOL + 1] - pq[2 * NCOL - 1];
+            dxw = pq[3 * NCOL + 1] - pq[3 * NCOL - 1];
+            dyu = pq[NCOL + RX] - pq[NCOL - RX];
+            dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
+            dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
+            const double* pmn = M.PB + M.pm * NP * NCOL + tc;
+            dzu = wn.u - pmn[NCOL]; dzv = wn.v - pmn[2 * NCOL]; dzw = wn.w - pmn[3 * NCOL];
+            M.GB[0 * NCOL + tc] = dyu; M.GB[1 * NCOL + tc] = dyv; M.GB[2 * NCOL + tc] = dzu; M.GB[3 * NCOL + tc] = dzw;
+            M.GB[4 * NCOL + tc] = dxv; M.GB[5 * NCOL + tc] = dxu; M.GB[6 * NCOL + tc] = dzv;
+        }
+    }
+    __syncthreads();                                              // (B) faces, differences (and prims q+1) visible
+
+    // ---------------- S3: acoustic update U~(q), PAPER.md:158-160 (+ reading A3 for the energy)
+    double Uc[5] = {0, 0, 0, 0, 0}, Ut[5] = {0, 0, 0, 0, 0};
+    double usxh = 0, pixh = 0, usyh = 0, piyh = 0, Six = 0, Siy = 0, Siz = 0;
+    ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
+    if (ROLE >= 1) {
+        const double* uc = M.UR + M.uq * 5 * NCOL + tc;
+        Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
+        usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1];
+        usyh = M.FB[2 * NCOL + tc + RX]; piyh = M.FB[3 * NCOL + tc + RX];
+        if (K.gx_on) Six = 0.5 * (fx.S + M.FB[4 * NCOL + tc + 1]);
+        if (K.gy_on) Siy = 0.5 * (fy.S + M.FB[5 * NCOL + tc + RX]);
+        Siz = 0.5 * (zhi.S + M.zlo.S);
+        const double sdu = (usxh - fx.us) + (usyh - fy.us) + (zhi.us - M.zlo.us);
+        const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us) + (zhi.pi * zhi.us - M.zlo.pi * M.zlo.us);
+        const double iLt = ark_rcp(1.0 + lam * sdu);
+        Ut[0] = Uc[0] * iLt;
+        Ut[1] = (Uc[1] - lam * (pixh - fx.pi) + lam * Six) * iLt;
+        Ut[2] = (Uc[2] - lam * (piyh - fy.pi) + lam * Siy) * iLt;
+        Ut[3] = (Uc[3] - lam * (zhi.pi - M.zlo.pi) + lam * Siz) * iLt;
+        Ut[4] = (Uc[4] - lam * sdpu) * iLt;
+        double* tb = M.TB + M.tq * 5 * NCOL + tc;
+        tb[0] = Ut[0]; tb[NCOL] = Ut[1]; tb[2 * NCOL] = Ut[2]; tb[3 * NCOL] = Ut[3]; tb[4 * NCOL] = Ut[4];
+
+        // viscous / heat fluxes through the low x, low y faces of plane q and the z face (q-1 | q)
+        if (VISC) {
+            const double Tc = pq[7 * NCOL];
+            if (do_update) {
+                if (ROLE == 2) {   // face (ci-1 | ci), normal x, transverse a = y, b = z
+                    const double* L = pq - 1;
+                    const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
+                    const int l = tc - 1;
+                    vx = ark_visc_face(K.KV, u - uL, v - vL, w - wL, M.GB[0 * NCOL + l] + dyu, M.GB[1 * NCOL + l] + dyv,
+                                       M.GB[2 * NCOL + l] + dzu, M.GB[3 * NCOL + l] + dzw, uL + u, vL + v, wL + w, Tc - TL);
+                    M.VB[0 * NCOL + tc] = vx.t0; M.VB[1 * NCOL + tc] = vx.t1; M.VB[2 * NCOL + tc] = vx.t2; M.VB[3 * NCOL + tc] = vx.fe;
+                }
+                {                  // face (cj-1 | cj), normal y, transverse a = x, b = z (row 1 computes it for nobody)
+                    const double* L = pq - RX;
+                    const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
+                    const int l = tc - RX;
+                    vy = ark_visc_face(K.KV, v - vL, u - uL, w - wL, M.GB[4 * NCOL + l] + dxv, M.GB[5 * NCOL + l] + dxu,
+                                       M.GB[6 * NCOL + l] + dzv, M.GB[3 * NCOL + l] + dzw, vL + v, uL + u, wL + w, Tc - TL);
+                    // stored as (tau_yx, tau_yy, tau_yz, fe): component order x,y,z
+                    M.VB[4 * NCOL + tc] = vy.t1; M.VB[5 * NCOL + tc] = vy.t0; M.VB[6 * NCOL + tc] = vy.t2; M.VB[7 * NCOL + tc] = vy.fe;
+                }
+            }
+            if (ROLE == 2) {
+                if (has_zlo) {     // face (q-1 | q), normal z, transverse a = x, b = y
+                    const double* pmn = M.PB + M.pm * NP * NCOL + tc;
+                    const double um = pmn[NCOL], vm = pmn[2 * NCOL], wm = pmn[3 * NCOL], Tm = pmn[7 * NCOL];
+                    vz = ark_visc_face(K.KV, w - wm, u - um, v - vm, M.gpz[0] + dxw, M.gpz[1] + dxu, M.gpz[2] + dyw, M.gpz[3] + dyv,
+                                       wm + w, um + u, vm + v, Tc - Tm);
+                }
+                M.gpz[0] = dxw; M.gpz[1] = dxu; M.gpz[2] = dyw; M.gpz[3] = dyv;
+            }
+        }
+    }
+    __syncthreads();                                              // (C) U~(q) and viscous fluxes visible
+
+    // ---------------- S4: transport + update
+    if (ROLE == 2) {
+        const double* Tq = M.TB + M.tq * 5 * NCOL;
+        double Gz[5] = {0, 0, 0, 0, 0};       // full flux through the z face (q-1|q)
+        double mzf = 0.0;
+        if (has_zlo) {
+            // upwind on u* (reading A10): U~(q-1) or U~(q) of the own column, both in the TB ring
+            const double* Tu = M.TB + (ark_nonneg(M.zlo.us) ? (M.tq ^ 1) : M.tq) * 5 * NCOL + tc;
+            const double zus = M.zlo.us, zpi = M.zlo.pi;
+            Gz[0] = Tu[0] * zus;
+            Gz[1] = Tu[NCOL] * zus;
+            Gz[2] = Tu[2 * NCOL] * zus;
+            Gz[3] = Tu[3 * NCOL] * zus + zpi;
+            Gz[4] = (Tu[4 * NCOL] + zpi) * zus;
+            mzf = Gz[0];
+            if (VISC) { Gz[1] -= vz.t1; Gz[2] -= vz.t2; Gz[3] -= vz.t0; Gz[4] -= vz.fe; }
+            if (completes) {
+                // complete and store U^{n+1}(q-1):  acc - lam * G_z(high) + gravity work of the high face
+                double out[5];
+                for (int f = 0; f < 5; ++f) out[f] = M.acc[f] - lam * Gz[f];
+                if (K.gz_on) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
+                if (M.inU) {
+                    double* __restrict__ c = M.Ocol + M.pstride * (long long)(q - 1);
+                    c[0] = out[0];
+                    c[M.fs] = out[1];
+                    c[2 * M.fs] = out[2];
+                    c[3 * M.fs] = out[3];
+                    c[4 * M.fs] = out[4];
+                }
+                if (M.want_rate) {
+                    const ark_u64 r = ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], K.inv_h, K.dcoef);
+                    M.rate_max = ark_umax(M.rate_max, M.inU ? r : 0ULL);
+                }
+            }
+        }
+        if (do_update) {
+            // in-plane faces of plane q: dG = sum_d (F_d+ - F_d-)
+            double dG[5];
+            double work = 0.0;
+            ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
+            ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
+            if (VISC) {
+                dG[1] -= (M.VB[0 * NCOL + tc + 1] - vx.t0) + (M.VB[4 * NCOL + tc + RX] - vy.t1);
+                dG[2] -= (M.VB[1 * NCOL + tc + 1] - vx.t1) + (M.VB[5 * NCOL + tc + RX] - vy.t0);
+                dG[3] -= (M.VB[2 * NCOL + tc + 1] - vx.t2) + (M.VB[6 * NCOL + tc + RX] - vy.t2);
+                dG[4] -= (M.VB[3 * NCOL + tc + 1] - vx.fe) + (M.VB[7 * NCOL + tc + RX] - vy.fe);
+            }
+            // low z face enters with +lam*G_z and the gravity work dt g_z max(m,0); the source lam*S_i
+            M.acc[0] = (Uc[0] - lam * dG[0]) + lam * Gz[0];
+            M.acc[1] = (Uc[1] - lam * dG[1] + lam * Six) + lam * Gz[1];
+            M.acc[2] = (Uc[2] - lam * dG[2] + lam * Siy) + lam * Gz[2];
+            M.acc[3] = (Uc[3] - lam * dG[3]) + lam * Gz[3];
+            M.acc[4] = (Uc[4] - lam * dG[4] + K.dt * work) + lam * Gz[4];
+            if (K.gz_on) {
+                M.acc[3] += lam * Siz;
+                M.acc[4] += K.dt * P.g[2] * ark_pos_part(mzf);
+            }
+        }
+    }
+    // rotate the rings
+    if (ROLE >= 1) M.zlo = zhi;
+    { const int s = M.uq; M.uq = M.un; M.un = M.unn; M.unn = s; }
+    if (VISC) { const int s = M.pm; M.pm = M.pc; M.pc = M.pn; M.pn = s; }
+    else      { const int s = M.pc; M.pc = M.pn; M.pn = s; }
+    M.tq ^= 1;
+}
+
+template <bool VISC, int TX, int TY, int ROLE>
+ARK_DEV void ark_march(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC, TX, TY>& M) {
+    int q = M.k0 - 1;
+    for (; q <= M.k0; ++q) ark_plane<VISC, TX, TY, ROLE, false>(P, K, M, q);    // k0-1, k0
+    for (; q < M.k1; ++q) ark_plane<VISC, TX, TY, ROLE, true>(P, K, M, q);      // k0+1 .. k1-1
+    for (; q <= M.k1; ++q) ark_plane<VISC, TX, TY, ROLE, false>(P, K, M, q);    // k1
+}
+
 template <bool VISC, int TX, int TY>
 ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
                         const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem) {
     using C = ArkStepCfg<3, VISC, TX, TY>;
     constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP, PSLOTS = C::PSLOTS;
-    double* UR = smem;                                // [3][5][NCOL]
-    double* PB = UR + 15 * NCOL;                      // [PSLOTS][NP][NCOL]
-    double* FB = PB + PSLOTS * NP * NCOL;             // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
-    double* TB = FB + 6 * NCOL;                       // [2][5][NCOL]: U~ of planes q-1, q
-    double* GB = TB + 10 * NCOL;                      // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
-    double* VB = GB + (VISC ? 7 : 0) * NCOL;          // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
-    ark_u64* red = (ark_u64*)(VB + (VISC ? 8 : 0) * NCOL);   // [32]
+    ArkMarch<VISC, TX, TY> M;
+    M.UR = smem;                                      // [3][5][NCOL]
+    M.PB = M.UR + 15 * NCOL;                          // [PSLOTS][NP][NCOL]
+    M.FB = M.PB + PSLOTS * NP * NCOL;                 // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
+    M.TB = M.FB + 6 * NCOL;                           // [2][5][NCOL]: U~ of planes q-1, q
+    M.GB = M.TB + 10 * NCOL;                          // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
+    M.VB = M.GB + (VISC ? 7 : 0) * NCOL;              // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
+    ark_u64* red = (ark_u64*)(M.VB + (VISC ? 8 : 0) * NCOL);   // [32]
 
     const int t = threadIdx.x;
     const int tc = t < NCOL ? t : NCOL - 1;
     const int ci = tc % RX, cj = tc / RX;
-    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-    const int gi = x0 - 2 + ci, gj = y0 - 2 + cj;      // interior-based cell coordinates of this column
+    const int gi = blockIdx.x * TX - 2 + ci, gj = blockIdx.y * TY - 2 + cj;   // interior-based cell coordinates
     // columns beyond the padded array (ragged tiles) load a valid cell; nobody consumes their results
     const int li = gi < P.nx + 2 ? gi : P.nx + 1;
     const int lj = gj < P.ny + 2 ? gj : P.ny + 1;
-    const int k0 = blockIdx.z * zchunk;
-    const int k1 = k0 + zchunk < P.nz ? k0 + zchunk : P.nz;
-
-    // roles: functions of the row only (warp-uniform when RX == 32)
-    const bool rowF = cj >= 1;                      // owns a low-y face
-    const bool rowA = cj >= 1 && cj <= RY - 2;      // tile + 1 ring: U~, centred differences
-    const bool rowU = cj >= 2 && cj <= RY - 3;      // tile: update
-    const bool rowVy = cj >= 2 && cj <= RY - 2;     // owns a viscous low-y face of the tile
-    const bool inU = t < NCOL && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;   // stores / rate only
+    M.tc = tc;
+    M.k0 = blockIdx.z * zchunk;
+    M.k1 = M.k0 + zchunk < P.nz ? M.k0 + zchunk : P.nz;
+    const bool rowA = cj >= 1 && cj <= RY - 2;      // tile + 1 ring
+    const bool rowU = cj >= 2 && cj <= RY - 3;      // tile
+    M.inU = t < NCOL && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;   // stores / rate only
+    M.want_rate = rate_scratch != nullptr;
 
     const ArkStepConst K = ark_step_const(P, dt_value, dt_dev);
-    const double lam = K.lam;
-
     const long long colbase = (long long)(li + ARK_XOFF) + (long long)P.px * (long long)(lj + ARK_NG);
-    const long long pstride = (long long)P.px * P.py;
-    const double* __restrict__ Ucol = Uin + colbase + pstride * (long long)P.offz;   // plane 0 of this column
-    double* __restrict__ Ocol = Uout + colbase + pstride * (long long)P.offz;
-    const long long fs = P.fstride;
+    M.pstride = (long long)P.px * P.py;
+    M.Ucol = Uin + colbase + M.pstride * (long long)P.offz;    // plane 0 of this column
+    M.Ocol = Uout + colbase + M.pstride * (long long)P.offz;
+    M.fs = P.fstride;
 
-    auto prefetch = [&](int k, int slot) {            // U^n(k) of the own column -> UR[slot]
-        const double* __restrict__ c = Ucol + pstride * (long long)k;
-        double* d = UR + slot * 5 * NCOL + tc;
-        ark_cp_async8(d, c);
-        ark_cp_async8(d + NCOL, c + fs);
-        ark_cp_async8(d + 2 * NCOL, c + 2 * fs);
-        ark_cp_async8(d + 3 * NCOL, c + 3 * fs);
-        ark_cp_async8(d + 4 * NCOL, c + 4 * fs);
-    };
-    auto primsOf = [&](int slot) {
-        const double* u = UR + slot * 5 * NCOL + tc;
-        return ark_prim_fast(P, u[0], u[NCOL], u[2 * NCOL], u[3 * NCOL], u[4 * NCOL]);
-    };
-    auto storePrim = [&](int slot, const ArkPrim& w) {
-        double* p = PB + slot * NP * NCOL + tc;
-        p[0] = w.rho; p[NCOL] = w.u; p[2 * NCOL] = w.v; p[3 * NCOL] = w.w;
-        p[4 * NCOL] = w.p; p[5 * NCOL] = w.rc; p[6 * NCOL] = w.irc;
-        if (VISC) p[7 * NCOL] = w.T;
-    };
-
-    // ring slots: UR by plane - (k0-2) mod 3; PB likewise (2 slots when the q-1 plane is not needed)
-    int uq = 1, un = 2, unn = 0;                   // planes q, q+1, q+2 at q = k0-1
-    int pm = 0, pc = VISC ? 1 : 0, pn = VISC ? 2 : 1;
-    int tq = 0;                                    // TB slot of plane q
+    // ring slots at q = k0-1: UR planes (k0-2,) k0-1, k0, k0+1 -> slots (0,) 1, 2, 0
+    M.uq = 1; M.un = 2; M.unn = 0;
+    M.pm = 0; M.pc = VISC ? 1 : 0; M.pn = VISC ? 2 : 1;
+    M.tq = 0;
 
     // ---- prologue: planes k0-2, k0-1 (and k0 in flight)
-    prefetch(k0 - 2, 0); ark_cp_async_commit();
-    prefetch(k0 - 1, 1); ark_cp_async_commit();
-    prefetch(k0, 2);     ark_cp_async_commit();
+    ark_march_prefetch(M, M.k0 - 2, 0); ark_cp_async_commit();
+    ark_march_prefetch(M, M.k0 - 1, 1); ark_cp_async_commit();
+    ark_march_prefetch(M, M.k0, 2);     ark_cp_async_commit();
     ark_cp_async_wait<1>();
-    ArkFace zlo;
     {
-        const ArkPrim wm = primsOf(0);
-        const ArkPrim wc0 = primsOf(1);
+        const ArkPrim wm = ark_march_prims(P, M, 0);
+        const ArkPrim wc0 = ark_march_prims(P, M, 1);
         if (VISC) {
-            double* p = PB + pm * NP * NCOL + tc;
+            double* p = M.PB + M.pm * NP * NCOL + tc;
             p[NCOL] = wm.u; p[2 * NCOL] = wm.v; p[3 * NCOL] = wm.w; p[7 * NCOL] = wm.T;
         }
-        storePrim(pc, wc0);
-        zlo = ark_face(K.th, K.ghz, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
+        double* p = M.PB + M.pc * NP * NCOL + tc;
+        p[0] = wc0.rho; p[NCOL] = wc0.u; p[2 * NCOL] = wc0.v; p[3 * NCOL] = wc0.w;
+        p[4 * NCOL] = wc0.p; p[5 * NCOL] = wc0.rc; p[6 * NCOL] = wc0.irc;
+        if (VISC) p[7 * NCOL] = wc0.T;
+        M.zlo = ark_face(K.th, K.ghz, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
     }
-    double acc[5] = {0, 0, 0, 0, 0};            // U^{n+1}(q-1) minus its high-z flux
-    double gpz[4] = {0, 0, 0, 0};               // dxw,dxu,dyw,dyv of the own column at q-1 (viscous z face)
-    ark_u64 rate_max = 0;
+    for (int f = 0; f < 5; ++f) M.acc[f] = 0.0;
+    for (int f = 0; f < 4; ++f) M.gpz[f] = 0.0;
+    M.rate_max = 0;
+    __syncthreads();                                  // primitives of plane k0-1 visible to the neighbours
 
-    for (int q = k0 - 1; q <= k1; ++q) {
-        // ---------------- S1: prefetch plane q+2, primitives of plane q+1
-        if (q + 2 <= k1 + 1) prefetch(q + 2, unn);
-        ark_cp_async_commit();
-        ark_cp_async_wait<1>();                                   // plane q+1 of the own column has landed
-        const ArkPrim wn = primsOf(un);
-        storePrim(pn, wn);
-        __syncthreads();                                          // (A) prims visible
-
-        const bool do_update = q >= k0 && q < k1;                 // plane q is an output plane of this chunk
-        // ---------------- S2: acoustic faces of plane q, centred velocity differences
-        const double* pq = PB + pc * NP * NCOL + tc;
-        double rho = 0, u = 0, v = 0, w = 0, p = 0, rc = 0, irc = 0;
-        ArkFace fx = {0, 0, 0}, fy = {0, 0, 0}, zhi = {0, 0, 0};
-        double dxu = 0, dxv = 0, dxw = 0, dyu = 0, dyv = 0, dyw = 0, dzu = 0, dzv = 0, dzw = 0;
-        if (rowF) {
-            rho = pq[0]; u = pq[NCOL]; v = pq[2 * NCOL]; w = pq[3 * NCOL]; p = pq[4 * NCOL]; rc = pq[5 * NCOL]; irc = pq[6 * NCOL];
-            {
-                const double* n = pq - RX;
-                fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
-                FB[2 * NCOL + tc] = fy.us; FB[3 * NCOL + tc] = fy.pi;
-                if (K.gy_on) FB[5 * NCOL + tc] = fy.S;
-            }
-            if (rowA) {
-                const double* n = pq - 1;
-                fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
-                FB[0 * NCOL + tc] = fx.us; FB[1 * NCOL + tc] = fx.pi;
-                if (K.gx_on) FB[4 * NCOL + tc] = fx.S;
-                zhi = ark_face(K.th, K.ghz, rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
-                if (VISC) {
-                    // un-normalised centred differences q(+1) - q(-1)
-                    dxu = pq[NCOL + 1] - pq[NCOL - 1];
-                    dxv = pq[2 * NCOL + 1] - pq[2 * NCOL - 1];
-                    dxw = pq[3 * NCOL + 1] - pq[3 * NCOL - 1];
-                    dyu = pq[NCOL + RX] - pq[NCOL - RX];
-                    dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
-                    dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
-                    const double* pmn = PB + pm * NP * NCOL + tc;
-                    dzu = wn.u - pmn[NCOL]; dzv = wn.v - pmn[2 * NCOL]; dzw = wn.w - pmn[3 * NCOL];
-                    GB[0 * NCOL + tc] = dyu; GB[1 * NCOL + tc] = dyv; GB[2 * NCOL + tc] = dzu; GB[3 * NCOL + tc] = dzw;
-                    GB[4 * NCOL + tc] = dxv; GB[5 * NCOL + tc] = dxu; GB[6 * NCOL + tc] = dzv;
-                }
-            }
-        }
-        __syncthreads();                                          // (B) faces and differences visible
-
-        // ---------------- S3: acoustic update U~(q), PAPER.md:158-160 (+ reading A3 for the energy)
-        double Uc[5] = {0, 0, 0, 0, 0}, Ut[5] = {0, 0, 0, 0, 0};
-        double usxh = 0, pixh = 0, usyh = 0, piyh = 0, Six = 0, Siy = 0, Siz = 0;
-        ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
-        if (rowA) {
-            const double* uc = UR + uq * 5 * NCOL + tc;
-            Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
-            usxh = FB[0 * NCOL + tc + 1]; pixh = FB[1 * NCOL + tc + 1];
-            usyh = FB[2 * NCOL + tc + RX]; piyh = FB[3 * NCOL + tc + RX];
-            if (K.gx_on) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
-            if (K.gy_on) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
-            Siz = 0.5 * (zhi.S + zlo.S);
-            const double sdu = (usxh - fx.us) + (usyh - fy.us) + (zhi.us - zlo.us);
-            const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us) + (zhi.pi * zhi.us - zlo.pi * zlo.us);
-            const double iLt = ark_rcp(1.0 + lam * sdu);
-            Ut[0] = Uc[0] * iLt;
-            Ut[1] = (Uc[1] - lam * (pixh - fx.pi) + lam * Six) * iLt;
-            Ut[2] = (Uc[2] - lam * (piyh - fy.pi) + lam * Siy) * iLt;
-            Ut[3] = (Uc[3] - lam * (zhi.pi - zlo.pi) + lam * Siz) * iLt;
-            Ut[4] = (Uc[4] - lam * sdpu) * iLt;
-            double* tb = TB + tq * 5 * NCOL + tc;
-            tb[0] = Ut[0]; tb[NCOL] = Ut[1]; tb[2 * NCOL] = Ut[2]; tb[3 * NCOL] = Ut[3]; tb[4 * NCOL] = Ut[4];
-        }
-        // viscous / heat fluxes through the low x, low y faces of plane q and the z face (q-1 | q)
-        if (VISC) {
-            if (rowVy) {
-                const double Tc = pq[7 * NCOL];
-                if (do_update) {
-                    if (rowU) {    // face (ci-1 | ci), normal x, transverse a = y, b = z
-                        const double* L = pq - 1;
-                        const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
-                        const int l = tc - 1;
-                        vx = ark_visc_face(K.KV, u - uL, v - vL, w - wL, GB[0 * NCOL + l] + dyu, GB[1 * NCOL + l] + dyv,
-                                           GB[2 * NCOL + l] + dzu, GB[3 * NCOL + l] + dzw, uL + u, vL + v, wL + w, Tc - TL);
-                        VB[0 * NCOL + tc] = vx.t0; VB[1 * NCOL + tc] = vx.t1; VB[2 * NCOL + tc] = vx.t2; VB[3 * NCOL + tc] = vx.fe;
-                    }
-                    {              // face (cj-1 | cj), normal y, transverse a = x, b = z
-                        const double* L = pq - RX;
-                        const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
-                        const int l = tc - RX;
-                        vy = ark_visc_face(K.KV, v - vL, u - uL, w - wL, GB[4 * NCOL + l] + dxv, GB[5 * NCOL + l] + dxu,
-                                           GB[6 * NCOL + l] + dzv, GB[3 * NCOL + l] + dzw, vL + v, uL + u, wL + w, Tc - TL);
-                        // stored as (tau_yx, tau_yy, tau_yz, fe): component order x,y,z
-                        VB[4 * NCOL + tc] = vy.t1; VB[5 * NCOL + tc] = vy.t0; VB[6 * NCOL + tc] = vy.t2; VB[7 * NCOL + tc] = vy.fe;
-                    }
-                }
-                if (rowU && q >= k0) {   // face (q-1 | q), normal z, transverse a = x, b = y
-                    const double* pmn = PB + pm * NP * NCOL + tc;
-                    const double um = pmn[NCOL], vm = pmn[2 * NCOL], wm = pmn[3 * NCOL], Tm = pmn[7 * NCOL];
-                    vz = ark_visc_face(K.KV, w - wm, u - um, v - vm, gpz[0] + dxw, gpz[1] + dxu, gpz[2] + dyw, gpz[3] + dyv,
-                                       wm + w, um + u, vm + v, Tc - Tm);
-                }
-            }
-            gpz[0] = dxw; gpz[1] = dxu; gpz[2] = dyw; gpz[3] = dyv;
-        }
-        __syncthreads();                                          // (C) U~(q) and viscous fluxes visible
-
-        // ---------------- S4: transport + update
-        if (rowU) {
-            const double* Tq = TB + tq * 5 * NCOL;
-            double Gz[5] = {0, 0, 0, 0, 0};       // full flux through the z face (q-1|q)
-            double mzf = 0.0;
-            if (q >= k0) {
-                const double* Tp = TB + (tq ^ 1) * 5 * NCOL + tc;     // U~(q-1), own column
-                if (ark_nonneg(zlo.us)) {                             // PAPER.md:174, reading A10
-                    for (int f = 0; f < 5; ++f) Gz[f] = Tp[f * NCOL] * zlo.us;
-                } else {
-                    for (int f = 0; f < 5; ++f) Gz[f] = Ut[f] * zlo.us;
-                }
-                mzf = Gz[0];
-                Gz[3] += zlo.pi;
-                Gz[4] += zlo.pi * zlo.us;
-                if (VISC) { Gz[1] -= vz.t1; Gz[2] -= vz.t2; Gz[3] -= vz.t0; Gz[4] -= vz.fe; }
-                if (q > k0) {
-                    // complete and store U^{n+1}(q-1):  acc - lam * G_z(high) + gravity work of the high face
-                    double out[5];
-                    for (int f = 0; f < 5; ++f) out[f] = acc[f] - lam * Gz[f];
-                    if (K.gz_on) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
-                    if (inU) {
-                        double* __restrict__ c = Ocol + pstride * (long long)(q - 1);
-                        c[0] = out[0];
-                        c[fs] = out[1];
-                        c[2 * fs] = out[2];
-                        c[3 * fs] = out[3];
-                        c[4 * fs] = out[4];
-                        if (rate_scratch) rate_max = ark_umax(rate_max, ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], K.inv_h, K.dcoef));
-                    }
-                }
-            }
-            if (do_update) {
-                // in-plane faces of plane q: dG = sum_d (F_d+ - F_d-)
-                double dG[5];
-                double work = 0.0;
-                ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
-                ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
-                if (VISC) {
-                    dG[1] -= (VB[0 * NCOL + tc + 1] - vx.t0) + (VB[4 * NCOL + tc + RX] - vy.t1);
-                    dG[2] -= (VB[1 * NCOL + tc + 1] - vx.t1) + (VB[5 * NCOL + tc + RX] - vy.t0);
-                    dG[3] -= (VB[2 * NCOL + tc + 1] - vx.t2) + (VB[6 * NCOL + tc + RX] - vy.t2);
-                    dG[4] -= (VB[3 * NCOL + tc + 1] - vx.fe) + (VB[7 * NCOL + tc + RX] - vy.fe);
-                }
-                // low z face enters with +lam*G_z and the gravity work dt g_z max(m,0); the source lam*S_i
-                acc[0] = (Uc[0] - lam * dG[0]) + lam * Gz[0];
-                acc[1] = (Uc[1] - lam * dG[1] + lam * Six) + lam * Gz[1];
-                acc[2] = (Uc[2] - lam * dG[2] + lam * Siy) + lam * Gz[2];
-                acc[3] = (Uc[3] - lam * dG[3]) + lam * Gz[3];
-                acc[4] = (Uc[4] - lam * dG[4] + K.dt * work) + lam * Gz[4];
-                if (K.gz_on) {
-                    acc[3] += lam * Siz;
-                    acc[4] += K.dt * P.g[2] * ark_pos_part(mzf);
-                }
-            }
-        }
-        // rotate the rings
-        zlo = zhi;
-        { const int s = uq; uq = un; un = unn; unn = s; }
-        if (VISC) { const int s = pm; pm = pc; pc = pn; pn = s; }
-        else      { const int s = pc; pc = pn; pn = s; }
-        tq ^= 1;
-    }
+    if (rowU)      ark_march<VISC, TX, TY, 2>(P, K, M);
+    else if (rowA) ark_march<VISC, TX, TY, 1>(P, K, M);
+    else           ark_march<VISC, TX, TY, 0>(P, K, M);
 
     if (rate_scratch) {
         // block-wide max of the rate bit patterns -> one double per block
-        ark_u64 m = rate_max;
+        ark_u64 m = M.rate_max;
 #ifndef ARK_HOST_EMU
         for (int o = 16; o > 0; o >>= 1) m = ark_umax(m, __shfl_xor_sync(0xffffffffu, m, o));
         const int lane = t & 31, wid = t >> 5;
