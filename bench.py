@@ -48,6 +48,44 @@ def build_workload(name, device=None, sample=False):
     return prm, U, bpc
 
 
+# fp64 ALU roof: 64 fp64 instructions / clk / SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
+# .peak_sustained = 64) x 148 SMs x clocks.max.sm 1965 MHz = 18.61 T fp64-instr/s (an FMA counts once).
+FP64_INSTR_PER_CLK_SM, N_SM, SM_MAX_MHZ = 64, 148, 1965.0
+# fp64 thread-instructions per cell update of the step kernel (halo recomputation included), from the committed ncu
+# capture of each kernel variant (profiles/): sum of DADD+DMUL+DFMA+DSETP warp instructions x 32 / cells.
+FP64_INSTR_PER_CELL = {"config5_512": 481.0, "config4_256": 481.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed `ncu --set full` capture
+DRAM_TRAFFIC_BYTES = {"config4_256": 1448.3e6}
+
+
+def max_over_ranks(x, dist=None, device=None):
+    """Time-like quantities are reduced with MAX over ranks (one all-reduce of one double, outside the timed region)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, ncell, steps, seconds):
+    """Replicas only: every rank advances its own copy of the workload; the job's throughput is the
+    cells all ranks updated divided by the slowest rank's time."""
+    return world * ncell * steps / seconds
+
+
+def fp64_roofline(workload, ncell, kern_ms):
+    """The viscous 3D step is fp64-ALU-bound before it is HBM-bound: second roofline object."""
+    ipc = FP64_INSTR_PER_CELL.get(workload)
+    if ipc is None:
+        return None
+    peak = FP64_INSTR_PER_CLK_SM * N_SM * SM_MAX_MHZ * 1e6 / 1e12
+    achieved = ipc * ncell / (kern_ms * 1e-3) / 1e12
+    return {"bound": "alu", "kernel": "ark_k_step", "achieved": achieved, "peak": peak, "unit": "T fp64-instr/s",
+            "frac": achieved / peak, "fp64_instr_per_cell": ipc,
+            "peak_source": "derived: 64 fp64 instr/clk/SM (ncu peak_sustained) x 148 SMs x 1965 MHz"}
+
+
 def measured_peaks():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
@@ -67,7 +105,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -190,11 +228,8 @@ def run_ours(args):
     kern_ms, kern_n = s.step_kernel_time()
     s.step_kernel_timing(False)
     launches = s.launch_count() - l0
-    if dist is not None:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * ncell * K / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ms_total, dist, dev)
+    value = whole_job_value(world, ncell, K, ms_total * 1e-3)
 
     # sanity: state still finite after the timed steps
     dt_chk = s.compute_dt(CFL)
@@ -216,11 +251,8 @@ def run_ours(args):
         s.get_state_host(host_out)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_val = world * ncell * e2e_steps / e2e_s
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
+    e2e_val = whole_job_value(world, ncell, e2e_steps, e2e_s)
 
     if rank == 0:
         peak, peak_src = measured_peaks()
@@ -237,10 +269,11 @@ def run_ours(args):
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "library": binding.version_string()},
                 "roofline": {"bound": "hbm", "kernel": "ark_k_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                             "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                             "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(args.workload), "peak_source": peak_src,
                              "algorithmic_bytes_per_cell": bpc, "kernel_ms": kern_avg_ms, "kernel_launches_timed": kern_n,
                              "kernel_share_of_step": kern_ms / ms_total,
                              "effective_whole_step_frac": bpc * value / world / 1e9 / peak},
+                "roofline_fp64": fp64_roofline(args.workload, ncell, kern_avg_ms),
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * 8,
                         "d2h_bytes_per_step": nfield * ncell * 8 + 16, "steps": e2e_steps,
                         "path": "ark_set_state_host + ark_compute_dt + ark_step + ark_get_state_host, pinned host buffers"},
@@ -257,7 +290,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5_512", choices=sorted(WORKLOADS))
