@@ -222,6 +222,7 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
         P.g[d] = d < ndim ? g[d] : 0.0;
         for (int sd = 0; sd < 2; ++sd) { P.bc[d][sd] = bc->type[d][sd]; P.bcv[d][sd] = bc->value[d][sd]; }
     }
+    ark_fill_derived(P);
     s->L = L;
     s->ws = (char*)d_workspace;
     s->U[0] = (double*)s->ws;
@@ -238,11 +239,17 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     // launch geometry of the fused step kernel
     if (ndim == 3) {
         const int gx = (nx + TX3 - 1) / TX3, gy = (ny + TY3 - 1) / TY3;
-        // z chunks: enough blocks for >= ~4 waves of 148 SMs, chunk length >= 16 planes (prologue = 2 planes)
-        int nchunk = 1;
-        while (nchunk < nz / 16 && (long long)gx * gy * nchunk < 148LL * 4) nchunk *= 2;
-        int zc = (nz + nchunk - 1) / nchunk;
-        nchunk = (nz + zc - 1) / zc;
+        // z chunks: a block marches zc planes (+ ~2.5 planes of prologue) and the grid runs in ceil(blocks / 148)
+        // rounds of one block per SM; pick the chunk count that minimises rounds * (zc + 2.5), chunks >= 16 planes
+        int zc = nz;
+        double best = 1e300;
+        for (int nch = 1; nch <= (nz / 16 > 1 ? nz / 16 : 1); ++nch) {
+            const int c = (nz + nch - 1) / nch;
+            const long long blocks = (long long)gx * gy * ((nz + c - 1) / c);
+            const double cost = (double)((blocks + 147) / 148) * (c + 2.5);
+            if (cost < best) { best = cost; zc = c; }
+        }
+        const int nchunk = (nz + zc - 1) / zc;
         s->zchunk = zc;
         s->step_grid = dim3(gx, gy, nchunk);
     } else {

@@ -27,6 +27,17 @@
 
 enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2 };
 
+// Coefficients of the dissipative face flux (see ark_visc_face in ark_step.cuh).
+struct ArkViscCoef { double cn, ct, c43, c23t, kh; };
+
+// Constants derived from the parameters on the host (ark_fill_derived).  They travel with ArkParams in the kernel
+// parameter (constant) bank, where fp64 instructions read them as operands: nothing uniform occupies a register.
+struct ArkDerived {
+    double inv_h, gh[3], dcoef;   // 1/h ; g_d h ; 2 ndim max(4 mu/3, (gamma-1) kappa) / h^2 (reading A4)
+    int g_on[3];
+    ArkViscCoef KV;
+};
+
 struct ArkParams {
     int nx, ny, nz, ndim, nf;   // interior sizes; nf = 4 (2D) or 5 (3D) stored fields
     int px, py, pz;             // padded extents (px is the row pitch)
@@ -36,7 +47,18 @@ struct ArkParams {
     int theta;                  // 0: theta == 1 ; 1: eq. (13)
     int bc[3][2];
     double bcv[3][2];
+    ArkDerived D;
 };
+
+inline void ark_fill_derived(ArkParams& P) {
+    ArkDerived& D = P.D;
+    D.inv_h = 1.0 / P.h;
+    for (int d = 0; d < 3; ++d) { D.gh[d] = P.g[d] * P.h; D.g_on[d] = D.gh[d] != 0.0; }
+    const double a = 4.0 * P.mu / 3.0, b = P.gm1 * P.kappa;
+    D.dcoef = 2.0 * P.ndim * (a > b ? a : b) * D.inv_h * D.inv_h;
+    D.KV.cn = P.mu * D.inv_h; D.KV.ct = 0.25 * P.mu * D.inv_h; D.KV.c43 = (4.0 / 3.0) * P.mu * D.inv_h;
+    D.KV.c23t = (2.0 / 3.0) * 0.25 * P.mu * D.inv_h; D.KV.kh = P.kappa * D.inv_h;
+}
 
 // padded linear index of interior-based cell (i,j,k); ghosts are -2,-1 and n,n+1
 ARK_DEV long long ark_idx(const ArkParams& P, int i, int j, int k) {

@@ -47,7 +47,7 @@ struct ArkStepCfg {
     static constexpr int TSLOTS = NDIM == 3 ? 2 : 1;
     // shared memory (doubles per column): UR, PB[PSLOTS][NP], FB[6], TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
     static constexpr int PER_COL = UR + PSLOTS * NP + 6 + TSLOTS * 5 + (VISC ? 15 : 0);
-    static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32;
+    static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32 + 16;   // + reduction + UR alignment pad
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
 };
 
@@ -57,9 +57,6 @@ struct ArkStepCfg {
 ARK_DEV bool ark_nonneg(double x) { return (int)(__double_as_longlong(x) >> 32) >= 0; }
 ARK_DEV double ark_pos_part(double x) { return ark_nonneg(x) ? x : 0.0; }   // max(x, 0)
 ARK_DEV double ark_neg_part(double x) { return ark_nonneg(x) ? 0.0 : x; }   // min(x, 0)
-
-// Coefficients of the dissipative face flux, precomputed once per thread.
-struct ArkViscCoef { double cn, ct, c43, c23t, kh; };
 
 struct ArkVisc { double t0, t1, t2, fe; };
 
@@ -98,25 +95,14 @@ ARK_DEV ark_u64 ark_rate_epilogue(const ArkParams& P, int ndim, double rho, doub
     return ark_rate_bits(r) & 0x7fffffffffffffffULL;
 }
 
-// per-thread constants of a step
-struct ArkStepConst {
-    double dt, lam, inv_h, ghx, ghy, ghz, dcoef;
-    bool gx_on, gy_on, gz_on;
-    int th;
-    ArkViscCoef KV;
-};
+// per-thread constants of a step: only the time step itself (it may come from device memory, ark_run); everything
+// else that is uniform sits in P.D (constant bank)
+struct ArkStepConst { double dt, lam; };
 
 ARK_DEV ArkStepConst ark_step_const(const ArkParams& P, double dt_value, const double* __restrict__ dt_dev) {
     ArkStepConst c;
     c.dt = dt_dev ? dt_dev[1] : dt_value;
-    c.inv_h = 1.0 / P.h;
     c.lam = c.dt / P.h;
-    c.ghx = P.g[0] * P.h; c.ghy = P.g[1] * P.h; c.ghz = P.g[2] * P.h;
-    c.gx_on = c.ghx != 0.0; c.gy_on = c.ghy != 0.0; c.gz_on = c.ghz != 0.0;
-    c.th = P.theta;
-    c.dcoef = 2.0 * P.ndim * fmax(4.0 * P.mu / 3.0, P.gm1 * P.kappa) * c.inv_h * c.inv_h;
-    c.KV.cn = P.mu * c.inv_h; c.KV.ct = 0.25 * P.mu * c.inv_h; c.KV.c43 = (4.0 / 3.0) * P.mu * c.inv_h;
-    c.KV.c23t = (2.0 / 3.0) * 0.25 * P.mu * c.inv_h; c.KV.kh = P.kappa * c.inv_h;
     return c;
 }
 
@@ -215,18 +201,18 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     ArkFace fy;
     {
         const double* n = pq - RX;
-        fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
+        fy = ark_face(P.theta, P.D.gh[1], n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
         M.FB[2 * NCOL + tc] = fy.us; M.FB[3 * NCOL + tc] = fy.pi;
-        if (K.gy_on) M.FB[5 * NCOL + tc] = fy.S;
+        if (P.D.g_on[1]) M.FB[5 * NCOL + tc] = fy.S;
     }
     ArkFace fx = fy, zhi = fy;                                    // (overwritten below for ROLE >= 1)
     double dxu = 0, dxv = 0, dxw = 0, dyu = 0, dyv = 0, dyw = 0, dzu = 0, dzv = 0, dzw = 0;
     if (ROLE >= 1) {
         const double* n = pq - 1;
-        fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
+        fx = ark_face(P.theta, P.D.gh[0], n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
         M.FB[0 * NCOL + tc] = fx.us; M.FB[1 * NCOL + tc] = fx.pi;
-        if (K.gx_on) M.FB[4 * NCOL + tc] = fx.S;
-        zhi = ark_face(K.th, K.ghz, rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
+        if (P.D.g_on[0]) M.FB[4 * NCOL + tc] = fx.S;
+        zhi = ark_face(P.theta, P.D.gh[2], rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
         if (VISC) {
             // un-normalised centred differences q(+1) - q(-1)
             dxu = pq[NCOL + 1] - pq[NCOL - 1];
@@ -252,8 +238,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
         Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
         usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1];
         usyh = M.FB[2 * NCOL + tc + RX]; piyh = M.FB[3 * NCOL + tc + RX];
-        if (K.gx_on) Six = 0.5 * (fx.S + M.FB[4 * NCOL + tc + 1]);
-        if (K.gy_on) Siy = 0.5 * (fy.S + M.FB[5 * NCOL + tc + RX]);
+        if (P.D.g_on[0]) Six = 0.5 * (fx.S + M.FB[4 * NCOL + tc + 1]);
+        if (P.D.g_on[1]) Siy = 0.5 * (fy.S + M.FB[5 * NCOL + tc + RX]);
         Siz = 0.5 * (zhi.S + M.zlo.S);
         const double sdu = (usxh - fx.us) + (usyh - fy.us) + (zhi.us - M.zlo.us);
         const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us) + (zhi.pi * zhi.us - M.zlo.pi * M.zlo.us);
@@ -274,7 +260,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                     const double* L = pq - 1;
                     const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
                     const int l = tc - 1;
-                    vx = ark_visc_face(K.KV, u - uL, v - vL, w - wL, M.GB[0 * NCOL + l] + dyu, M.GB[1 * NCOL + l] + dyv,
+                    vx = ark_visc_face(P.D.KV, u - uL, v - vL, w - wL, M.GB[0 * NCOL + l] + dyu, M.GB[1 * NCOL + l] + dyv,
                                        M.GB[2 * NCOL + l] + dzu, M.GB[3 * NCOL + l] + dzw, uL + u, vL + v, wL + w, Tc - TL);
                     M.VB[0 * NCOL + tc] = vx.t0; M.VB[1 * NCOL + tc] = vx.t1; M.VB[2 * NCOL + tc] = vx.t2; M.VB[3 * NCOL + tc] = vx.fe;
                 }
@@ -282,7 +268,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                     const double* L = pq - RX;
                     const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
                     const int l = tc - RX;
-                    vy = ark_visc_face(K.KV, v - vL, u - uL, w - wL, M.GB[4 * NCOL + l] + dxv, M.GB[5 * NCOL + l] + dxu,
+                    vy = ark_visc_face(P.D.KV, v - vL, u - uL, w - wL, M.GB[4 * NCOL + l] + dxv, M.GB[5 * NCOL + l] + dxu,
                                        M.GB[6 * NCOL + l] + dzv, M.GB[3 * NCOL + l] + dzw, vL + v, uL + u, wL + w, Tc - TL);
                     // stored as (tau_yx, tau_yy, tau_yz, fe): component order x,y,z
                     M.VB[4 * NCOL + tc] = vy.t1; M.VB[5 * NCOL + tc] = vy.t0; M.VB[6 * NCOL + tc] = vy.t2; M.VB[7 * NCOL + tc] = vy.fe;
@@ -292,7 +278,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                 if (has_zlo) {     // face (q-1 | q), normal z, transverse a = x, b = y
                     const double* pmn = M.PB + M.pm * NP * NCOL + tc;
                     const double um = pmn[NCOL], vm = pmn[2 * NCOL], wm = pmn[3 * NCOL], Tm = pmn[7 * NCOL];
-                    vz = ark_visc_face(K.KV, w - wm, u - um, v - vm, M.gpz[0] + dxw, M.gpz[1] + dxu, M.gpz[2] + dyw, M.gpz[3] + dyv,
+                    vz = ark_visc_face(P.D.KV, w - wm, u - um, v - vm, M.gpz[0] + dxw, M.gpz[1] + dxu, M.gpz[2] + dyw, M.gpz[3] + dyv,
                                        wm + w, um + u, vm + v, Tc - Tm);
                 }
                 M.gpz[0] = dxw; M.gpz[1] = dxu; M.gpz[2] = dyw; M.gpz[3] = dyv;
@@ -321,7 +307,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                 // complete and store U^{n+1}(q-1):  acc - lam * G_z(high) + gravity work of the high face
                 double out[5];
                 for (int f = 0; f < 5; ++f) out[f] = M.acc[f] - lam * Gz[f];
-                if (K.gz_on) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
+                if (P.D.g_on[2]) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
                 if (M.inU) {
                     double* __restrict__ c = M.Ocol + M.pstride * (long long)(q - 1);
                     c[0] = out[0];
@@ -331,7 +317,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                     c[4 * M.fs] = out[4];
                 }
                 if (M.want_rate) {
-                    const ark_u64 r = ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], K.inv_h, K.dcoef);
+                    const ark_u64 r = ark_rate_epilogue(P, 3, out[0], out[1], out[2], out[3], out[4], P.D.inv_h, P.D.dcoef);
                     M.rate_max = ark_umax(M.rate_max, M.inU ? r : 0ULL);
                 }
             }
@@ -340,8 +326,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             // in-plane faces of plane q: dG = sum_d (F_d+ - F_d-)
             double dG[5];
             double work = 0.0;
-            ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
-            ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
+            ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, P.D.g_on[0], P.g[0], dG, work, true);
+            ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, P.D.g_on[1], P.g[1], dG, work, false);
             if (VISC) {
                 dG[1] -= (M.VB[0 * NCOL + tc + 1] - vx.t0) + (M.VB[4 * NCOL + tc + RX] - vy.t1);
                 dG[2] -= (M.VB[1 * NCOL + tc + 1] - vx.t1) + (M.VB[5 * NCOL + tc + RX] - vy.t0);
@@ -354,7 +340,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             M.acc[2] = (Uc[2] - lam * dG[2] + lam * Siy) + lam * Gz[2];
             M.acc[3] = (Uc[3] - lam * dG[3]) + lam * Gz[3];
             M.acc[4] = (Uc[4] - lam * dG[4] + K.dt * work) + lam * Gz[4];
-            if (K.gz_on) {
+            if (P.D.g_on[2]) {
                 M.acc[3] += lam * Siz;
                 M.acc[4] += K.dt * P.g[2] * ark_pos_part(mzf);
             }
@@ -382,8 +368,10 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     using C = ArkStepCfg<3, VISC, TX, TY>;
     constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP, PSLOTS = C::PSLOTS;
     ArkMarch<VISC, TX, TY> M;
-    M.UR = smem;                                      // [3][5][NCOL]
-    M.PB = M.UR + 15 * NCOL;                          // [PSLOTS][NP][NCOL]
+    // the UR ring starts at the same offset modulo 128 bytes as the tile's rows in global memory (row pitch, plane and
+    // field strides are multiples of 128 B), so that every 32-byte sector of a cp.async lands sector-aligned
+    M.UR = smem + ((blockIdx.x * TX + ARK_XOFF - 2) & 15);   // [3][5][NCOL]
+    M.PB = smem + 16 + 15 * NCOL;                     // [PSLOTS][NP][NCOL]
     M.FB = M.PB + PSLOTS * NP * NCOL;                 // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
     M.TB = M.FB + 6 * NCOL;                           // [2][5][NCOL]: U~ of planes q-1, q
     M.GB = M.TB + 10 * NCOL;                          // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
@@ -433,7 +421,7 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
         p[0] = wc0.rho; p[NCOL] = wc0.u; p[2 * NCOL] = wc0.v; p[3 * NCOL] = wc0.w;
         p[4 * NCOL] = wc0.p; p[5 * NCOL] = wc0.rc; p[6 * NCOL] = wc0.irc;
         if (VISC) p[7 * NCOL] = wc0.T;
-        M.zlo = ark_face(K.th, K.ghz, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
+        M.zlo = ark_face(P.theta, P.D.gh[2], wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
     }
     for (int f = 0; f < 5; ++f) M.acc[f] = 0.0;
     for (int f = 0; f < 4; ++f) M.gpz[f] = 0.0;
@@ -513,15 +501,15 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
     if (rowF) {
         {
             const double* n = pq - RX;
-            fy = ark_face(K.th, K.ghy, n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.v, wc.p, wc.rc, wc.irc);
+            fy = ark_face(P.theta, P.D.gh[1], n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.v, wc.p, wc.rc, wc.irc);
             FB[2 * NCOL + tc] = fy.us; FB[3 * NCOL + tc] = fy.pi;
-            if (K.gy_on) FB[5 * NCOL + tc] = fy.S;
+            if (P.D.g_on[1]) FB[5 * NCOL + tc] = fy.S;
         }
         if (rowA) {
             const double* n = pq - 1;
-            fx = ark_face(K.th, K.ghx, n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.u, wc.p, wc.rc, wc.irc);
+            fx = ark_face(P.theta, P.D.gh[0], n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], wc.rho, wc.u, wc.p, wc.rc, wc.irc);
             FB[0 * NCOL + tc] = fx.us; FB[1 * NCOL + tc] = fx.pi;
-            if (K.gx_on) FB[4 * NCOL + tc] = fx.S;
+            if (P.D.g_on[0]) FB[4 * NCOL + tc] = fx.S;
             if (VISC) {
                 dxu = pq[NCOL + 1] - pq[NCOL - 1];
                 dxv = pq[2 * NCOL + 1] - pq[2 * NCOL - 1];
@@ -538,8 +526,8 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
     if (rowA) {
         usxh = FB[0 * NCOL + tc + 1]; pixh = FB[1 * NCOL + tc + 1];
         usyh = FB[2 * NCOL + tc + RX]; piyh = FB[3 * NCOL + tc + RX];
-        if (K.gx_on) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
-        if (K.gy_on) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
+        if (P.D.g_on[0]) Six = 0.5 * (fx.S + FB[4 * NCOL + tc + 1]);
+        if (P.D.g_on[1]) Siy = 0.5 * (fy.S + FB[5 * NCOL + tc + RX]);
         const double sdu = (usxh - fx.us) + (usyh - fy.us);
         const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us);
         const double iLt = ark_rcp(1.0 + lam * sdu);
@@ -554,7 +542,7 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
             const double* L = pq - 1;
             const double uL = L[NCOL], vL = L[2 * NCOL], TL = L[7 * NCOL];
             const int l = tc - 1;
-            vx = ark_visc_face(K.KV, wc.u - uL, wc.v - vL, 0.0, GB[0 * NCOL + l] + dyu, GB[1 * NCOL + l] + dyv, 0.0, 0.0,
+            vx = ark_visc_face(P.D.KV, wc.u - uL, wc.v - vL, 0.0, GB[0 * NCOL + l] + dyu, GB[1 * NCOL + l] + dyv, 0.0, 0.0,
                                uL + wc.u, vL + wc.v, 0.0, wc.T - TL);
             VB[0 * NCOL + tc] = vx.t0; VB[1 * NCOL + tc] = vx.t1; VB[3 * NCOL + tc] = vx.fe;
         }
@@ -562,7 +550,7 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
             const double* L = pq - RX;
             const double uL = L[NCOL], vL = L[2 * NCOL], TL = L[7 * NCOL];
             const int l = tc - RX;
-            vy = ark_visc_face(K.KV, wc.v - vL, wc.u - uL, 0.0, GB[4 * NCOL + l] + dxv, GB[5 * NCOL + l] + dxu, 0.0, 0.0,
+            vy = ark_visc_face(P.D.KV, wc.v - vL, wc.u - uL, 0.0, GB[4 * NCOL + l] + dxv, GB[5 * NCOL + l] + dxu, 0.0, 0.0,
                                vL + wc.v, uL + wc.u, 0.0, wc.T - TL);
             VB[4 * NCOL + tc] = vy.t1; VB[5 * NCOL + tc] = vy.t0; VB[7 * NCOL + tc] = vy.fe;
         }
@@ -573,8 +561,8 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
     if (rowU) {
         double dG[5];
         double work = 0.0;
-        ark_transport_axis<2, 1>(TB, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, K.gx_on, P.g[0], dG, work, true);
-        ark_transport_axis<2, 2>(TB, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, K.gy_on, P.g[1], dG, work, false);
+        ark_transport_axis<2, 1>(TB, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, P.D.g_on[0], P.g[0], dG, work, true);
+        ark_transport_axis<2, 2>(TB, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, P.D.g_on[1], P.g[1], dG, work, false);
         if (VISC) {
             dG[1] -= (VB[0 * NCOL + tc + 1] - vx.t0) + (VB[4 * NCOL + tc + RX] - vy.t1);
             dG[2] -= (VB[1 * NCOL + tc + 1] - vx.t1) + (VB[5 * NCOL + tc + RX] - vy.t0);
@@ -586,7 +574,7 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
         const double n4 = Uc[4] - lam * dG[4] + K.dt * work;
         if (inU) {
             Uout[colbase] = n0; Uout[colbase + fs] = n1; Uout[colbase + 2 * fs] = n2; Uout[colbase + 3 * fs] = n4;
-            if (rate_scratch) rate_max = ark_rate_epilogue(P, 2, n0, n1, n2, 0.0, n4, K.inv_h, K.dcoef);
+            if (rate_scratch) rate_max = ark_rate_epilogue(P, 2, n0, n1, n2, 0.0, n4, P.D.inv_h, P.D.dcoef);
         }
     }
     if (rate_scratch) {

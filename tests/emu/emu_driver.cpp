@@ -23,6 +23,7 @@ ArkParams make_params(int nx, int ny, int nz, double h, double gamma, const doub
         P.g[d] = d < P.ndim ? g[d] : 0.0;
         for (int s = 0; s < 2; ++s) { P.bc[d][s] = bt[2 * d + s]; P.bcv[d][s] = bv[2 * d + s]; }
     }
+    ark_fill_derived(P);
     return P;
 }
 
