@@ -12,7 +12,7 @@ LIB = os.path.join(HERE, "libark_b200.so")
 SOURCES = ["ark.cu"]
 HEADERS = ["ark_device.cuh", "ark_step.cuh", os.path.join("..", "..", "include", "ark.h")]
 # tile of the fused step kernel: (TX, TY) outputs per block and plane, region (TX+4) x (TY+4) threads
-TILES = {"ARK_TX3": 28, "ARK_TY3": 8, "ARK_TX2": 28, "ARK_TY2": 8}
+TILES = {"ARK_TX3": 28, "ARK_TY3": 10, "ARK_TX2": 28, "ARK_TY2": 8}
 
 
 def nvcc_cmd(out, extra=()):

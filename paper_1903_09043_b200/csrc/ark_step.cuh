@@ -40,13 +40,18 @@
 template <int NDIM, bool VISC, int TX, int TY>
 struct ArkStepCfg {
     static constexpr int RX = TX + 4, RY = TY + 4, NCOL = RX * RY;
-    static constexpr int NT = ((NCOL + 31) / 32) * 32;
+    // 3D: one thread per column of rows 1..RY-2; the two edge rows 0 and RY-1 (primitives only) are the second
+    // column of the threads of the ring rows 1 and RY-2, whose own work is light.  2D: one thread per column.
+    static constexpr int NTHR = NDIM == 3 ? RX * (RY - 2) : NCOL;
+    static constexpr int NT = ((NTHR + 31) / 32) * 32;
     static constexpr int NP = VISC ? 8 : 7;                          // T only feeds the heat flux
-    static constexpr int PSLOTS = NDIM == 3 ? (VISC ? 3 : 2) : 1;    // plane q-1 only feeds the viscous z stencil
+    static constexpr int PSLOTS = NDIM == 3 ? 2 : 1;                 // primitives of planes q, q+1
+    static constexpr int PM = NDIM == 3 && VISC ? 4 : 0;             // u,v,w,T of plane q-1 (viscous z stencil)
     static constexpr int UR = NDIM == 3 ? 15 : 0;                    // [3][5]
+    static constexpr int FBN = NDIM == 3 ? 4 : 6;                    // 3D recomputes the gravity face terms S
     static constexpr int TSLOTS = NDIM == 3 ? 2 : 1;
-    // shared memory (doubles per column): UR, PB[PSLOTS][NP], FB[6], TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
-    static constexpr int PER_COL = UR + PSLOTS * NP + 6 + TSLOTS * 5 + (VISC ? 15 : 0);
+    // shared memory (doubles per column): UR, PB[PSLOTS][NP], PM, FB, TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
+    static constexpr int PER_COL = UR + PSLOTS * NP + PM + FBN + TSLOTS * 5 + (VISC ? 15 : 0);
     static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32 + 16;   // + reduction + UR alignment pad
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
 };
@@ -132,21 +137,23 @@ ARK_DEV void ark_transport_axis(const double* __restrict__ T, int cs, int tc, in
 // 3D body.  The march is specialised by ROW ROLE (a compile-time parameter of the whole plane loop, chosen once
 // per thread and warp-uniform when RX == 32) so that no role test, no predicate and no dummy initialisation is
 // left inside an iteration:
-//   ROLE 0  edge rows 0, RY-1 : primitives, low-y acoustic face
-//   ROLE 1  ring rows 1, RY-2 : + low-x / high-z faces, centred differences, U~, viscous low-y face
+//   ROLE 1  ring rows 1, RY-2 : primitives, acoustic faces, centred differences, U~, viscous low-y face; each thread
+//                               also keeps the primitives of the EDGE row next to it (row 0 / RY-1: prefetch,
+//                               primitives and, for row RY-1, its low-y face) -- the edge rows have no threads
 //   ROLE 2  tile rows 2..RY-3 : + viscous x / z faces, transport, update, store, CFL rate
 // and by STEADY (planes k0+1 .. k1-1, where every chunk-boundary condition is known) vs. the generic first and
 // last iterations.  Every role executes the same two barriers per plane.
 // ------------------------------------------------------------------------------------------------------------
 template <bool VISC, int TX, int TY>
 struct ArkMarch {
-    double *UR, *PB, *FB, *TB, *GB, *VB;
+    double *UR, *PB, *PM, *FB, *TB, *GB, *VB;
     const double* Ucol;
+    const double* Ucol2;                 // ring rows: the edge column (row 0 or RY-1) this thread also serves
     double* Ocol;
     long long pstride, fs;
-    int tc, k0, k1;
-    bool inU, want_rate;
-    int uq, un, unn, pm, pc, pn, tq;     // ring slots of planes q, q+1, q+2 (UR); q-1, q, q+1 (PB); q (TB)
+    int tc, tc2, k0, k1;
+    bool inU, want_rate, top;            // top: ring row RY-2 (its edge row RY-1 owns a low-y face)
+    int uq, un, unn, pc, pn, tq;         // ring slots of planes q, q+1, q+2 (UR); q, q+1 (PB); q (TB)
     ArkFace zlo;                         // acoustic z face (q-1|q)
     double acc[5];                       // U^{n+1}(q-1) minus its high-z flux
     double gpz[4];                       // dxw,dxu,dyw,dyv of the own column at q-1 (viscous z face)
@@ -154,10 +161,11 @@ struct ArkMarch {
 };
 
 template <bool VISC, int TX, int TY>
-ARK_DEV void ark_march_prefetch(const ArkMarch<VISC, TX, TY>& M, int k, int slot) {   // U^n(k), own column -> UR[slot]
+ARK_DEV void ark_march_prefetch(const ArkMarch<VISC, TX, TY>& M, const double* __restrict__ col, int tc, int k, int slot) {
+    // U^n(k) of one column -> UR[slot]
     constexpr int NCOL = ArkStepCfg<3, VISC, TX, TY>::NCOL;
-    const double* __restrict__ c = M.Ucol + M.pstride * (long long)k;
-    double* d = M.UR + slot * 5 * NCOL + M.tc;
+    const double* __restrict__ c = col + M.pstride * (long long)k;
+    double* d = M.UR + slot * 5 * NCOL + tc;
     ark_cp_async8(d, c);
     ark_cp_async8(d + NCOL, c + M.fs);
     ark_cp_async8(d + 2 * NCOL, c + 2 * M.fs);
@@ -166,9 +174,18 @@ ARK_DEV void ark_march_prefetch(const ArkMarch<VISC, TX, TY>& M, int k, int slot
 }
 
 template <bool VISC, int TX, int TY>
-ARK_DEV ArkPrim ark_march_prims(const ArkParams& P, const ArkMarch<VISC, TX, TY>& M, int slot) {
+ARK_DEV void ark_store_prims(const ArkMarch<VISC, TX, TY>& M, int slot, int tc, const ArkPrim& w) {
+    using C = ArkStepCfg<3, VISC, TX, TY>;
+    double* p = M.PB + slot * C::NP * C::NCOL + tc;
+    p[0] = w.rho; p[C::NCOL] = w.u; p[2 * C::NCOL] = w.v; p[3 * C::NCOL] = w.w;
+    p[4 * C::NCOL] = w.p; p[5 * C::NCOL] = w.rc; p[6 * C::NCOL] = w.irc;
+    if (VISC) p[7 * C::NCOL] = w.T;
+}
+
+template <bool VISC, int TX, int TY>
+ARK_DEV ArkPrim ark_march_prims(const ArkParams& P, const ArkMarch<VISC, TX, TY>& M, int tc, int slot) {
     constexpr int NCOL = ArkStepCfg<3, VISC, TX, TY>::NCOL;
-    const double* u = M.UR + slot * 5 * NCOL + M.tc;
+    const double* u = M.UR + slot * 5 * NCOL + tc;
     return ark_prim_fast(P, u[0], u[NCOL], u[2 * NCOL], u[3 * NCOL], u[4 * NCOL]);
 }
 
@@ -183,16 +200,15 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     const bool completes = STEADY || q > M.k0;                    // plane q-1 is completed and stored here
 
     // ---------------- S1: prefetch plane q+2, primitives of plane q+1 (own column)
-    if (STEADY || q + 2 <= M.k1 + 1) ark_march_prefetch(M, q + 2, M.unn);
-    ark_cp_async_commit();
-    ark_cp_async_wait<1>();                                       // plane q+1 of the own column has landed
-    const ArkPrim wn = ark_march_prims(P, M, M.un);
-    {
-        double* p = M.PB + M.pn * NP * NCOL + tc;
-        p[0] = wn.rho; p[NCOL] = wn.u; p[2 * NCOL] = wn.v; p[3 * NCOL] = wn.w;
-        p[4 * NCOL] = wn.p; p[5 * NCOL] = wn.rc; p[6 * NCOL] = wn.irc;
-        if (VISC) p[7 * NCOL] = wn.T;
+    if (STEADY || q + 2 <= M.k1 + 1) {
+        ark_march_prefetch(M, M.Ucol, tc, q + 2, M.unn);
+        if (ROLE == 1) ark_march_prefetch(M, M.Ucol2, M.tc2, q + 2, M.unn);
     }
+    ark_cp_async_commit();
+    ark_cp_async_wait<1>();                                       // plane q+1 of the own column(s) has landed
+    const ArkPrim wn = ark_march_prims(P, M, tc, M.un);
+    ark_store_prims(M, M.pn, tc, wn);
+    if (ROLE == 1) ark_store_prims(M, M.pn, M.tc2, ark_march_prims(P, M, M.tc2, M.un));
     // (no barrier: S2 reads the neighbours' primitives of plane q, written one iteration ago)
 
     // ---------------- S2: acoustic faces of plane q, centred velocity differences
@@ -203,15 +219,18 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
         const double* n = pq - RX;
         fy = ark_face(P.theta, P.D.gh[1], n[0], n[2 * NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, v, p, rc, irc);
         M.FB[2 * NCOL + tc] = fy.us; M.FB[3 * NCOL + tc] = fy.pi;
-        if (P.D.g_on[1]) M.FB[5 * NCOL + tc] = fy.S;
     }
-    ArkFace fx = fy, zhi = fy;                                    // (overwritten below for ROLE >= 1)
+    if (ROLE == 1 && M.top) {                                     // low-y face of the edge row RY-1 (own cell | edge cell)
+        const double* e = pq + RX;
+        const ArkFace f2 = ark_face(P.theta, P.D.gh[1], rho, v, p, rc, irc, e[0], e[2 * NCOL], e[4 * NCOL], e[5 * NCOL], e[6 * NCOL]);
+        M.FB[2 * NCOL + M.tc2] = f2.us; M.FB[3 * NCOL + M.tc2] = f2.pi;
+    }
+    ArkFace fx, zhi;
     double dxu = 0, dxv = 0, dxw = 0, dyu = 0, dyv = 0, dyw = 0, dzu = 0, dzv = 0, dzw = 0;
-    if (ROLE >= 1) {
+    {
         const double* n = pq - 1;
         fx = ark_face(P.theta, P.D.gh[0], n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
         M.FB[0 * NCOL + tc] = fx.us; M.FB[1 * NCOL + tc] = fx.pi;
-        if (P.D.g_on[0]) M.FB[4 * NCOL + tc] = fx.S;
         zhi = ark_face(P.theta, P.D.gh[2], rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
         if (VISC) {
             // un-normalised centred differences q(+1) - q(-1)
@@ -221,8 +240,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             dyu = pq[NCOL + RX] - pq[NCOL - RX];
             dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
             dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
-            const double* pmn = M.PB + M.pm * NP * NCOL + tc;
-            dzu = wn.u - pmn[NCOL]; dzv = wn.v - pmn[2 * NCOL]; dzw = wn.w - pmn[3 * NCOL];
+            const double* pmn = M.PM + tc;
+            dzu = wn.u - pmn[0]; dzv = wn.v - pmn[NCOL]; dzw = wn.w - pmn[2 * NCOL];
             M.GB[0 * NCOL + tc] = dyu; M.GB[1 * NCOL + tc] = dyv; M.GB[2 * NCOL + tc] = dzu; M.GB[3 * NCOL + tc] = dzw;
             M.GB[4 * NCOL + tc] = dxv; M.GB[5 * NCOL + tc] = dxu; M.GB[6 * NCOL + tc] = dzv;
         }
@@ -233,13 +252,14 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     double Uc[5] = {0, 0, 0, 0, 0}, Ut[5] = {0, 0, 0, 0, 0};
     double usxh = 0, pixh = 0, usyh = 0, piyh = 0, Six = 0, Siy = 0, Siz = 0;
     ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
-    if (ROLE >= 1) {
+    {
         const double* uc = M.UR + M.uq * 5 * NCOL + tc;
         Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
         usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1];
         usyh = M.FB[2 * NCOL + tc + RX]; piyh = M.FB[3 * NCOL + tc + RX];
-        if (P.D.g_on[0]) Six = 0.5 * (fx.S + M.FB[4 * NCOL + tc + 1]);
-        if (P.D.g_on[1]) Siy = 0.5 * (fy.S + M.FB[5 * NCOL + tc + RX]);
+        // S_i = (S_low + S_high)/2; the high face's S is recomputed exactly as its owner computes it
+        if (P.D.g_on[0]) Six = 0.5 * (fx.S + (0.5 * P.D.gh[0]) * (rho + pq[1]));
+        if (P.D.g_on[1]) Siy = 0.5 * (fy.S + (0.5 * P.D.gh[1]) * (rho + pq[RX]));
         Siz = 0.5 * (zhi.S + M.zlo.S);
         const double sdu = (usxh - fx.us) + (usyh - fy.us) + (zhi.us - M.zlo.us);
         const double sdpu = (pixh * usxh - fx.pi * fx.us) + (piyh * usyh - fy.pi * fy.us) + (zhi.pi * zhi.us - M.zlo.pi * M.zlo.us);
@@ -276,13 +296,16 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             }
             if (ROLE == 2) {
                 if (has_zlo) {     // face (q-1 | q), normal z, transverse a = x, b = y
-                    const double* pmn = M.PB + M.pm * NP * NCOL + tc;
-                    const double um = pmn[NCOL], vm = pmn[2 * NCOL], wm = pmn[3 * NCOL], Tm = pmn[7 * NCOL];
+                    const double* pmn = M.PM + tc;
+                    const double um = pmn[0], vm = pmn[NCOL], wm = pmn[2 * NCOL], Tm = pmn[3 * NCOL];
                     vz = ark_visc_face(P.D.KV, w - wm, u - um, v - vm, M.gpz[0] + dxw, M.gpz[1] + dxu, M.gpz[2] + dyw, M.gpz[3] + dyv,
                                        wm + w, um + u, vm + v, Tc - Tm);
                 }
                 M.gpz[0] = dxw; M.gpz[1] = dxu; M.gpz[2] = dyw; M.gpz[3] = dyv;
             }
+            // plane q becomes plane q-1 of the next iteration (own column only: no hazard)
+            double* pmw = M.PM + tc;
+            pmw[0] = u; pmw[NCOL] = v; pmw[2 * NCOL] = w; pmw[3 * NCOL] = Tc;
         }
     }
     __syncthreads();                                              // (C) U~(q) and viscous fluxes visible
@@ -347,10 +370,9 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
         }
     }
     // rotate the rings
-    if (ROLE >= 1) M.zlo = zhi;
+    M.zlo = zhi;
     { const int s = M.uq; M.uq = M.un; M.un = M.unn; M.unn = s; }
-    if (VISC) { const int s = M.pm; M.pm = M.pc; M.pc = M.pn; M.pn = s; }
-    else      { const int s = M.pc; M.pc = M.pn; M.pn = s; }
+    { const int s = M.pc; M.pc = M.pn; M.pn = s; }
     M.tq ^= 1;
 }
 
@@ -366,20 +388,22 @@ template <bool VISC, int TX, int TY>
 ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
                         const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem) {
     using C = ArkStepCfg<3, VISC, TX, TY>;
-    constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP, PSLOTS = C::PSLOTS;
+    constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP;
     ArkMarch<VISC, TX, TY> M;
     // the UR ring starts at the same offset modulo 128 bytes as the tile's rows in global memory (row pitch, plane and
     // field strides are multiples of 128 B), so that every 32-byte sector of a cp.async lands sector-aligned
     M.UR = smem + ((blockIdx.x * TX + ARK_XOFF - 2) & 15);   // [3][5][NCOL]
-    M.PB = smem + 16 + 15 * NCOL;                     // [PSLOTS][NP][NCOL]
-    M.FB = M.PB + PSLOTS * NP * NCOL;                 // [6][NCOL]: usx,pix,usy,piy,Sx,Sy (low faces of plane q)
-    M.TB = M.FB + 6 * NCOL;                           // [2][5][NCOL]: U~ of planes q-1, q
+    M.PB = smem + 16 + 15 * NCOL;                     // [2][NP][NCOL]
+    M.PM = M.PB + 2 * NP * NCOL;                      // [4][NCOL]: u,v,w,T of plane q-1 (VISC)
+    M.FB = M.PM + C::PM * NCOL;                       // [4][NCOL]: usx,pix,usy,piy (low faces of plane q)
+    M.TB = M.FB + 4 * NCOL;                           // [2][5][NCOL]: U~ of planes q-1, q
     M.GB = M.TB + 10 * NCOL;                          // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
     M.VB = M.GB + (VISC ? 7 : 0) * NCOL;              // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
     ark_u64* red = (ark_u64*)(M.VB + (VISC ? 8 : 0) * NCOL);   // [32]
 
+    // thread -> column of rows 1..RY-2 (one warp per row when RX == 32)
     const int t = threadIdx.x;
-    const int tc = t < NCOL ? t : NCOL - 1;
+    const int tc = (t < C::NTHR ? t : C::NTHR - 1) + RX;
     const int ci = tc % RX, cj = tc / RX;
     const int gi = blockIdx.x * TX - 2 + ci, gj = blockIdx.y * TY - 2 + cj;   // interior-based cell coordinates
     // columns beyond the padded array (ragged tiles) load a valid cell; nobody consumes their results
@@ -388,39 +412,44 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.tc = tc;
     M.k0 = blockIdx.z * zchunk;
     M.k1 = M.k0 + zchunk < P.nz ? M.k0 + zchunk : P.nz;
-    const bool rowA = cj >= 1 && cj <= RY - 2;      // tile + 1 ring
-    const bool rowU = cj >= 2 && cj <= RY - 3;      // tile
-    M.inU = t < NCOL && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;   // stores / rate only
+    const bool rowU = cj >= 2 && cj <= RY - 3;      // tile rows; the others (1, RY-2) are the ring
+    M.inU = t < C::NTHR && rowU && ci >= 2 && ci < 2 + TX && gi < P.nx && gj < P.ny;   // stores / rate only
     M.want_rate = rate_scratch != nullptr;
+    // ring rows also serve the edge row next to them (row 0 below row 1, row RY-1 above row RY-2)
+    M.top = cj == RY - 2;
+    M.tc2 = M.top ? tc + RX : tc - RX;
+    const int gj2 = M.top ? gj + 1 : gj - 1;
+    const int lj2 = gj2 < P.ny + 2 ? gj2 : P.ny + 1;
 
     const ArkStepConst K = ark_step_const(P, dt_value, dt_dev);
     const long long colbase = (long long)(li + ARK_XOFF) + (long long)P.px * (long long)(lj + ARK_NG);
     M.pstride = (long long)P.px * P.py;
     M.Ucol = Uin + colbase + M.pstride * (long long)P.offz;    // plane 0 of this column
+    M.Ucol2 = M.Ucol + (long long)P.px * (long long)(lj2 - lj);
     M.Ocol = Uout + colbase + M.pstride * (long long)P.offz;
     M.fs = P.fstride;
 
     // ring slots at q = k0-1: UR planes (k0-2,) k0-1, k0, k0+1 -> slots (0,) 1, 2, 0
     M.uq = 1; M.un = 2; M.unn = 0;
-    M.pm = 0; M.pc = VISC ? 1 : 0; M.pn = VISC ? 2 : 1;
+    M.pc = 0; M.pn = 1;
     M.tq = 0;
 
     // ---- prologue: planes k0-2, k0-1 (and k0 in flight)
-    ark_march_prefetch(M, M.k0 - 2, 0); ark_cp_async_commit();
-    ark_march_prefetch(M, M.k0 - 1, 1); ark_cp_async_commit();
-    ark_march_prefetch(M, M.k0, 2);     ark_cp_async_commit();
+    for (int s3 = 0; s3 < 3; ++s3) {
+        ark_march_prefetch(M, M.Ucol, tc, M.k0 - 2 + s3, s3);
+        if (!rowU) ark_march_prefetch(M, M.Ucol2, M.tc2, M.k0 - 2 + s3, s3);
+        ark_cp_async_commit();
+    }
     ark_cp_async_wait<1>();
     {
-        const ArkPrim wm = ark_march_prims(P, M, 0);
-        const ArkPrim wc0 = ark_march_prims(P, M, 1);
+        const ArkPrim wm = ark_march_prims(P, M, tc, 0);
+        const ArkPrim wc0 = ark_march_prims(P, M, tc, 1);
         if (VISC) {
-            double* p = M.PB + M.pm * NP * NCOL + tc;
-            p[NCOL] = wm.u; p[2 * NCOL] = wm.v; p[3 * NCOL] = wm.w; p[7 * NCOL] = wm.T;
+            double* p = M.PM + tc;
+            p[0] = wm.u; p[NCOL] = wm.v; p[2 * NCOL] = wm.w; p[3 * NCOL] = wm.T;
         }
-        double* p = M.PB + M.pc * NP * NCOL + tc;
-        p[0] = wc0.rho; p[NCOL] = wc0.u; p[2 * NCOL] = wc0.v; p[3 * NCOL] = wc0.w;
-        p[4 * NCOL] = wc0.p; p[5 * NCOL] = wc0.rc; p[6 * NCOL] = wc0.irc;
-        if (VISC) p[7 * NCOL] = wc0.T;
+        ark_store_prims(M, M.pc, tc, wc0);
+        if (!rowU) ark_store_prims(M, M.pc, M.tc2, ark_march_prims(P, M, M.tc2, 1));
         M.zlo = ark_face(P.theta, P.D.gh[2], wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
     }
     for (int f = 0; f < 5; ++f) M.acc[f] = 0.0;
@@ -428,9 +457,8 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.rate_max = 0;
     __syncthreads();                                  // primitives of plane k0-1 visible to the neighbours
 
-    if (rowU)      ark_march<VISC, TX, TY, 2>(P, K, M);
-    else if (rowA) ark_march<VISC, TX, TY, 1>(P, K, M);
-    else           ark_march<VISC, TX, TY, 0>(P, K, M);
+    if (rowU) ark_march<VISC, TX, TY, 2>(P, K, M);
+    else      ark_march<VISC, TX, TY, 1>(P, K, M);
 
     if (rate_scratch) {
         // block-wide max of the rate bit patterns -> one double per block
