@@ -111,26 +111,37 @@ ARK_DEV double ark_rsqrt(double x) {
 #endif
 }
 
-// 8-byte asynchronous global -> shared copies (LDGSTS): the U^n prefetch ring of the 3D step kernel.
-ARK_DEV void ark_cp_async8(double* smem_dst, const double* gsrc) {
+// TMA bulk copies global -> shared (cp.async.bulk, SASS UBLKCP) completing on an mbarrier: the U^n prefetch ring of
+// the 3D step kernel.  One elected lane issues whole 256-byte rows; the data never passes through registers or the
+// LSU pipe of the issuing warp.  (Host emulation: see ark_step.cuh, the copies are done synchronously per thread.)
 #ifndef ARK_HOST_EMU
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
-#else
-    *smem_dst = *gsrc;
-#endif
+ARK_DEV unsigned ark_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+ARK_DEV void ark_mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ark_smem_u32(bar)), "r"(count) : "memory");
 }
-ARK_DEV void ark_cp_async_commit() {
-#ifndef ARK_HOST_EMU
-    asm volatile("cp.async.commit_group;" ::: "memory");
-#endif
+ARK_DEV void ark_mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
-template <int N>
-ARK_DEV void ark_cp_async_wait() {
-#ifndef ARK_HOST_EMU
-    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
-#endif
+ARK_DEV void ark_mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ark_smem_u32(bar)), "r"(bytes) : "memory");
 }
+ARK_DEV void ark_bulk_g2s(double* smem_dst, const double* gsrc, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(ark_smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(ark_smem_u32(bar)) : "memory");
+}
+ARK_DEV void ark_mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "ARK_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra ARK_DONE_%=;\n"
+        "bra ARK_WAIT_%=;\n"
+        "ARK_DONE_%=:\n"
+        "}\n" ::"r"(ark_smem_u32(bar)), "r"(parity) : "memory");
+}
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // Primitive variables of one cell (PAPER.md:315-319 ideal gas, c^2 = gamma p / rho; :370 p = rho T).

@@ -46,13 +46,12 @@ struct ArkStepCfg {
     static constexpr int NT = ((NTHR + 31) / 32) * 32;
     static constexpr int NP = VISC ? 8 : 7;                          // T only feeds the heat flux
     static constexpr int PSLOTS = NDIM == 3 ? 2 : 1;                 // primitives of planes q, q+1
-    static constexpr int PM = NDIM == 3 && VISC ? 4 : 0;             // u,v,w,T of plane q-1 (viscous z stencil)
     static constexpr int UR = NDIM == 3 ? 15 : 0;                    // [3][5]
     static constexpr int FBN = NDIM == 3 ? 4 : 6;                    // 3D recomputes the gravity face terms S
     static constexpr int TSLOTS = NDIM == 3 ? 2 : 1;
-    // shared memory (doubles per column): UR, PB[PSLOTS][NP], PM, FB, TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
-    static constexpr int PER_COL = UR + PSLOTS * NP + PM + FBN + TSLOTS * 5 + (VISC ? 15 : 0);
-    static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32 + 16;   // + reduction + UR alignment pad
+    // shared memory (doubles per column): UR, PB[PSLOTS][NP], FB, TB[TSLOTS][5], GB[7], VB[8] (+ 32 for the reduction)
+    static constexpr int PER_COL = UR + PSLOTS * NP + FBN + TSLOTS * 5 + (VISC ? 15 : 0);
+    static constexpr int SMEM_DOUBLES = PER_COL * NCOL + 32 + 3 * RY;   // + reduction + per row: 3 mbarriers (UR slots), phase counter
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
 };
 
@@ -146,31 +145,65 @@ ARK_DEV void ark_transport_axis(const double* __restrict__ T, int cs, int tc, in
 // ------------------------------------------------------------------------------------------------------------
 template <bool VISC, int TX, int TY>
 struct ArkMarch {
-    double *UR, *PB, *PM, *FB, *TB, *GB, *VB;
+    double *UR, *PB, *FB, *TB, *GB, *VB;
     const double* Ucol;
     const double* Ucol2;                 // ring rows: the edge column (row 0 or RY-1) this thread also serves
+    const double *Urow, *Urow2;          // column 0 of the own row / of the edge row (TMA bulk copies of whole rows)
+    unsigned long long* mbar;            // the row's three mbarriers (one per UR slot)
+    unsigned phase;                      // parity bit of each slot's next completion
+    int row0, row2;                      // first column index of the own row / the edge row
+    bool leader;                         // lane 0 of the row: issues the copies
     double* Ocol;
     long long pstride, fs;
     int tc, tc2, k0, k1;
     bool inU, want_rate, top;            // top: ring row RY-2 (its edge row RY-1 owns a low-y face)
     int uq, un, unn, pc, pn, tq;         // ring slots of planes q, q+1, q+2 (UR); q, q+1 (PB); q (TB)
+    ArkPrim wc;                          // primitives of the own column at plane q
+    double wm[4];                        // u,v,w,T of the own column at plane q-1 (viscous z stencil)
     ArkFace zlo;                         // acoustic z face (q-1|q)
     double acc[5];                       // U^{n+1}(q-1) minus its high-z flux
     double gpz[4];                       // dxw,dxu,dyw,dyv of the own column at q-1 (viscous z face)
     ark_u64 rate_max;
 };
 
+// U^n(k) of this thread's row(s) -> UR[slot].  GPU: lane 0 of the row's warp issues one 256-byte TMA bulk copy per
+// field (and the same for the edge row a ring warp serves), all completing on the warp's mbarrier of that slot.
+// Host emulation: every thread copies its own column(s) synchronously.
 template <bool VISC, int TX, int TY>
-ARK_DEV void ark_march_prefetch(const ArkMarch<VISC, TX, TY>& M, const double* __restrict__ col, int tc, int k, int slot) {
-    // U^n(k) of one column -> UR[slot]
-    constexpr int NCOL = ArkStepCfg<3, VISC, TX, TY>::NCOL;
-    const double* __restrict__ c = col + M.pstride * (long long)k;
-    double* d = M.UR + slot * 5 * NCOL + tc;
-    ark_cp_async8(d, c);
-    ark_cp_async8(d + NCOL, c + M.fs);
-    ark_cp_async8(d + 2 * NCOL, c + 2 * M.fs);
-    ark_cp_async8(d + 3 * NCOL, c + 3 * M.fs);
-    ark_cp_async8(d + 4 * NCOL, c + 4 * M.fs);
+ARK_DEV void ark_ring_issue(const ArkMarch<VISC, TX, TY>& M, int k, int slot, bool edge) {
+    using C = ArkStepCfg<3, VISC, TX, TY>;
+    constexpr int NCOL = C::NCOL;
+#ifndef ARK_HOST_EMU
+    if (M.leader) {
+        constexpr unsigned ROWB = C::RX * sizeof(double);
+        unsigned long long* bar = M.mbar + slot;
+        ark_mbar_expect_tx(bar, (edge ? 10u : 5u) * ROWB);
+        const double* __restrict__ c = M.Urow + M.pstride * (long long)k;
+        double* d = M.UR + slot * 5 * NCOL + M.row0;
+        for (int f = 0; f < 5; ++f) ark_bulk_g2s(d + f * NCOL, c + f * M.fs, ROWB, bar);
+        if (edge) {
+            const double* __restrict__ c2 = M.Urow2 + M.pstride * (long long)k;
+            double* d2 = M.UR + slot * 5 * NCOL + M.row2;
+            for (int f = 0; f < 5; ++f) ark_bulk_g2s(d2 + f * NCOL, c2 + f * M.fs, ROWB, bar);
+        }
+    }
+#else
+    for (int e = 0; e < (edge ? 2 : 1); ++e) {
+        const double* c = (e ? M.Ucol2 : M.Ucol) + M.pstride * (long long)k;
+        double* d = M.UR + slot * 5 * NCOL + (e ? M.tc2 : M.tc);
+        for (int f = 0; f < 5; ++f) d[f * NCOL] = c[f * M.fs];
+    }
+#endif
+}
+
+template <bool VISC, int TX, int TY>
+ARK_DEV void ark_ring_wait(ArkMarch<VISC, TX, TY>& M, int slot) {
+#ifndef ARK_HOST_EMU
+    ark_mbar_wait(M.mbar + slot, (M.phase >> slot) & 1u);
+    M.phase ^= 1u << slot;
+#else
+    (void)M; (void)slot;
+#endif
 }
 
 template <bool VISC, int TX, int TY>
@@ -200,12 +233,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     const bool completes = STEADY || q > M.k0;                    // plane q-1 is completed and stored here
 
     // ---------------- S1: prefetch plane q+2, primitives of plane q+1 (own column)
-    if (STEADY || q + 2 <= M.k1 + 1) {
-        ark_march_prefetch(M, M.Ucol, tc, q + 2, M.unn);
-        if (ROLE == 1) ark_march_prefetch(M, M.Ucol2, M.tc2, q + 2, M.unn);
-    }
-    ark_cp_async_commit();
-    ark_cp_async_wait<1>();                                       // plane q+1 of the own column(s) has landed
+    if (STEADY || q + 2 <= M.k1 + 1) ark_ring_issue(M, q + 2, M.unn, ROLE == 1);
+    ark_ring_wait(M, M.un);                                       // plane q+1 of the own row(s) has landed
     const ArkPrim wn = ark_march_prims(P, M, tc, M.un);
     ark_store_prims(M, M.pn, tc, wn);
     if (ROLE == 1) ark_store_prims(M, M.pn, M.tc2, ark_march_prims(P, M, M.tc2, M.un));
@@ -213,7 +242,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
 
     // ---------------- S2: acoustic faces of plane q, centred velocity differences
     const double* pq = M.PB + M.pc * NP * NCOL + tc;
-    const double rho = pq[0], u = pq[NCOL], v = pq[2 * NCOL], w = pq[3 * NCOL], p = pq[4 * NCOL], rc = pq[5 * NCOL], irc = pq[6 * NCOL];
+    const double rho = M.wc.rho, u = M.wc.u, v = M.wc.v, w = M.wc.w, p = M.wc.p, rc = M.wc.rc, irc = M.wc.irc;
     ArkFace fy;
     {
         const double* n = pq - RX;
@@ -240,8 +269,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             dyu = pq[NCOL + RX] - pq[NCOL - RX];
             dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
             dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
-            const double* pmn = M.PM + tc;
-            dzu = wn.u - pmn[0]; dzv = wn.v - pmn[NCOL]; dzw = wn.w - pmn[2 * NCOL];
+            dzu = wn.u - M.wm[0]; dzv = wn.v - M.wm[1]; dzw = wn.w - M.wm[2];
             M.GB[0 * NCOL + tc] = dyu; M.GB[1 * NCOL + tc] = dyv; M.GB[2 * NCOL + tc] = dzu; M.GB[3 * NCOL + tc] = dzw;
             M.GB[4 * NCOL + tc] = dxv; M.GB[5 * NCOL + tc] = dxu; M.GB[6 * NCOL + tc] = dzv;
         }
@@ -254,7 +282,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     ArkVisc vx = {0, 0, 0, 0}, vy = {0, 0, 0, 0}, vz = {0, 0, 0, 0};
     {
         const double* uc = M.UR + M.uq * 5 * NCOL + tc;
-        Uc[0] = uc[0]; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
+        Uc[0] = rho; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
         usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1];
         usyh = M.FB[2 * NCOL + tc + RX]; piyh = M.FB[3 * NCOL + tc + RX];
         // S_i = (S_low + S_high)/2; the high face's S is recomputed exactly as its owner computes it
@@ -274,7 +302,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
 
         // viscous / heat fluxes through the low x, low y faces of plane q and the z face (q-1 | q)
         if (VISC) {
-            const double Tc = pq[7 * NCOL];
+            const double Tc = M.wc.T;
             if (do_update) {
                 if (ROLE == 2) {   // face (ci-1 | ci), normal x, transverse a = y, b = z
                     const double* L = pq - 1;
@@ -296,16 +324,12 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             }
             if (ROLE == 2) {
                 if (has_zlo) {     // face (q-1 | q), normal z, transverse a = x, b = y
-                    const double* pmn = M.PM + tc;
-                    const double um = pmn[0], vm = pmn[NCOL], wm = pmn[2 * NCOL], Tm = pmn[3 * NCOL];
+                    const double um = M.wm[0], vm = M.wm[1], wm = M.wm[2], Tm = M.wm[3];
                     vz = ark_visc_face(P.D.KV, w - wm, u - um, v - vm, M.gpz[0] + dxw, M.gpz[1] + dxu, M.gpz[2] + dyw, M.gpz[3] + dyv,
                                        wm + w, um + u, vm + v, Tc - Tm);
                 }
                 M.gpz[0] = dxw; M.gpz[1] = dxu; M.gpz[2] = dyw; M.gpz[3] = dyv;
             }
-            // plane q becomes plane q-1 of the next iteration (own column only: no hazard)
-            double* pmw = M.PM + tc;
-            pmw[0] = u; pmw[NCOL] = v; pmw[2 * NCOL] = w; pmw[3 * NCOL] = Tc;
         }
     }
     __syncthreads();                                              // (C) U~(q) and viscous fluxes visible
@@ -371,6 +395,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     }
     // rotate the rings
     M.zlo = zhi;
+    if (VISC) { M.wm[0] = u; M.wm[1] = v; M.wm[2] = w; M.wm[3] = M.wc.T; }
+    M.wc = wn;
     { const int s = M.uq; M.uq = M.un; M.un = M.unn; M.unn = s; }
     { const int s = M.pc; M.pc = M.pn; M.pn = s; }
     M.tq ^= 1;
@@ -390,16 +416,14 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     using C = ArkStepCfg<3, VISC, TX, TY>;
     constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP;
     ArkMarch<VISC, TX, TY> M;
-    // the UR ring starts at the same offset modulo 128 bytes as the tile's rows in global memory (row pitch, plane and
-    // field strides are multiples of 128 B), so that every 32-byte sector of a cp.async lands sector-aligned
-    M.UR = smem + ((blockIdx.x * TX + ARK_XOFF - 2) & 15);   // [3][5][NCOL]
-    M.PB = smem + 16 + 15 * NCOL;                     // [2][NP][NCOL]
-    M.PM = M.PB + 2 * NP * NCOL;                      // [4][NCOL]: u,v,w,T of plane q-1 (VISC)
-    M.FB = M.PM + C::PM * NCOL;                       // [4][NCOL]: usx,pix,usy,piy (low faces of plane q)
+    M.UR = smem;                                      // [3][5][NCOL]
+    M.PB = smem + 15 * NCOL;                          // [2][NP][NCOL]
+    M.FB = M.PB + 2 * NP * NCOL;                      // [4][NCOL]: usx,pix,usy,piy (low faces of plane q)
     M.TB = M.FB + 4 * NCOL;                           // [2][5][NCOL]: U~ of planes q-1, q
     M.GB = M.TB + 10 * NCOL;                          // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
     M.VB = M.GB + (VISC ? 7 : 0) * NCOL;              // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
     ark_u64* red = (ark_u64*)(M.VB + (VISC ? 8 : 0) * NCOL);   // [32]
+    unsigned long long* mbars = red + 32;             // [RY-2][3]
 
     // thread -> column of rows 1..RY-2 (one warp per row when RX == 32)
     const int t = threadIdx.x;
@@ -428,6 +452,22 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.Ucol2 = M.Ucol + (long long)P.px * (long long)(lj2 - lj);
     M.Ocol = Uout + colbase + M.pstride * (long long)P.offz;
     M.fs = P.fstride;
+    // whole rows for the bulk copies start at region column 0 (never clamped in x: a ragged tile's row runs on into
+    // the padding / the next row, valid memory whose values nobody consumes)
+    M.Urow = M.Ucol - (li - (int)(blockIdx.x * TX - 2));
+    M.Urow2 = M.Ucol2 - (li - (int)(blockIdx.x * TX - 2));
+    M.row0 = cj * RX;
+    M.row2 = M.top ? M.row0 + RX : M.row0 - RX;
+    M.leader = ci == 0;
+    M.mbar = mbars + 3 * (cj - 1);
+    M.phase = 0;
+#ifndef ARK_HOST_EMU
+    if (M.leader) {
+        for (int s3 = 0; s3 < 3; ++s3) ark_mbar_init(M.mbar + s3, 1);
+        ark_mbar_fence_init();
+    }
+    __syncthreads();
+#endif
 
     // ring slots at q = k0-1: UR planes (k0-2,) k0-1, k0, k0+1 -> slots (0,) 1, 2, 0
     M.uq = 1; M.un = 2; M.unn = 0;
@@ -435,19 +475,14 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.tq = 0;
 
     // ---- prologue: planes k0-2, k0-1 (and k0 in flight)
-    for (int s3 = 0; s3 < 3; ++s3) {
-        ark_march_prefetch(M, M.Ucol, tc, M.k0 - 2 + s3, s3);
-        if (!rowU) ark_march_prefetch(M, M.Ucol2, M.tc2, M.k0 - 2 + s3, s3);
-        ark_cp_async_commit();
-    }
-    ark_cp_async_wait<1>();
+    for (int s3 = 0; s3 < 3; ++s3) ark_ring_issue(M, M.k0 - 2 + s3, s3, !rowU);
+    ark_ring_wait(M, 0);
+    ark_ring_wait(M, 1);
     {
         const ArkPrim wm = ark_march_prims(P, M, tc, 0);
         const ArkPrim wc0 = ark_march_prims(P, M, tc, 1);
-        if (VISC) {
-            double* p = M.PM + tc;
-            p[0] = wm.u; p[NCOL] = wm.v; p[2 * NCOL] = wm.w; p[3 * NCOL] = wm.T;
-        }
+        M.wm[0] = wm.u; M.wm[1] = wm.v; M.wm[2] = wm.w; M.wm[3] = wm.T;
+        M.wc = wc0;
         ark_store_prims(M, M.pc, tc, wc0);
         if (!rowU) ark_store_prims(M, M.pc, M.tc2, ark_march_prims(P, M, M.tc2, 1));
         M.zlo = ark_face(P.theta, P.D.gh[2], wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0.rho, wc0.w, wc0.p, wc0.rc, wc0.irc);
