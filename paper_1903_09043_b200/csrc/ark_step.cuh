@@ -64,6 +64,19 @@ ARK_DEV double ark_neg_part(double x) { return ark_nonneg(x) ? 0.0 : x; }   // m
 
 struct ArkVisc { double t0, t1, t2, fe; };
 
+// Exchange with the x neighbours by warp shuffle when a region row is exactly one warp (RX == 32): what only the
+// left / right neighbour consumes (high-x acoustic face, the left cell's centred differences, the high-x viscous
+// flux) then never touches shared memory.  Other tile widths and the host emulation use the shared arrays.
+#ifndef ARK_HOST_EMU
+#define ARK_XSHFL(RX) ((RX) == 32)
+ARK_DEV double ark_from_left(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+ARK_DEV double ark_from_right(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+#else
+#define ARK_XSHFL(RX) false
+ARK_DEV double ark_from_left(double v) { return v; }
+ARK_DEV double ark_from_right(double v) { return v; }
+#endif
+
 // Dissipative flux through a face with unit normal along axis d (tau = mu(grad u + grad u^T)
 // + eta div u I, eta = -2/3 mu; divergence form, Fourier flux; stencil = reading A6).
 //   dn_*  : (u_d, u_a, u_b)_R - (..)_L                        normal differences (un-normalised)
@@ -259,7 +272,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     {
         const double* n = pq - 1;
         fx = ark_face(P.theta, P.D.gh[0], n[0], n[NCOL], n[4 * NCOL], n[5 * NCOL], n[6 * NCOL], rho, u, p, rc, irc);
-        M.FB[0 * NCOL + tc] = fx.us; M.FB[1 * NCOL + tc] = fx.pi;
+        if (!ARK_XSHFL(RX)) { M.FB[0 * NCOL + tc] = fx.us; M.FB[1 * NCOL + tc] = fx.pi; }
         zhi = ark_face(P.theta, P.D.gh[2], rho, w, p, rc, irc, wn.rho, wn.w, wn.p, wn.rc, wn.irc);
         if (VISC) {
             // un-normalised centred differences q(+1) - q(-1)
@@ -270,7 +283,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             dyv = pq[2 * NCOL + RX] - pq[2 * NCOL - RX];
             dyw = pq[3 * NCOL + RX] - pq[3 * NCOL - RX];
             dzu = wn.u - M.wm[0]; dzv = wn.v - M.wm[1]; dzw = wn.w - M.wm[2];
-            M.GB[0 * NCOL + tc] = dyu; M.GB[1 * NCOL + tc] = dyv; M.GB[2 * NCOL + tc] = dzu; M.GB[3 * NCOL + tc] = dzw;
+            if (!ARK_XSHFL(RX)) { M.GB[0 * NCOL + tc] = dyu; M.GB[1 * NCOL + tc] = dyv; M.GB[2 * NCOL + tc] = dzu; }
+            M.GB[3 * NCOL + tc] = dzw;
             M.GB[4 * NCOL + tc] = dxv; M.GB[5 * NCOL + tc] = dxu; M.GB[6 * NCOL + tc] = dzv;
         }
     }
@@ -283,7 +297,8 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
     {
         const double* uc = M.UR + M.uq * 5 * NCOL + tc;
         Uc[0] = rho; Uc[1] = uc[NCOL]; Uc[2] = uc[2 * NCOL]; Uc[3] = uc[3 * NCOL]; Uc[4] = uc[4 * NCOL];
-        usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1];
+        if (ARK_XSHFL(RX)) { usxh = ark_from_right(fx.us); pixh = ark_from_right(fx.pi); }
+        else               { usxh = M.FB[0 * NCOL + tc + 1]; pixh = M.FB[1 * NCOL + tc + 1]; }
         usyh = M.FB[2 * NCOL + tc + RX]; piyh = M.FB[3 * NCOL + tc + RX];
         // S_i = (S_low + S_high)/2; the high face's S is recomputed exactly as its owner computes it
         if (P.D.g_on[0]) Six = 0.5 * (fx.S + (0.5 * P.D.gh[0]) * (rho + pq[1]));
@@ -308,9 +323,14 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                     const double* L = pq - 1;
                     const double uL = L[NCOL], vL = L[2 * NCOL], wL = L[3 * NCOL], TL = L[7 * NCOL];
                     const int l = tc - 1;
-                    vx = ark_visc_face(P.D.KV, u - uL, v - vL, w - wL, M.GB[0 * NCOL + l] + dyu, M.GB[1 * NCOL + l] + dyv,
-                                       M.GB[2 * NCOL + l] + dzu, M.GB[3 * NCOL + l] + dzw, uL + u, vL + v, wL + w, Tc - TL);
-                    M.VB[0 * NCOL + tc] = vx.t0; M.VB[1 * NCOL + tc] = vx.t1; M.VB[2 * NCOL + tc] = vx.t2; M.VB[3 * NCOL + tc] = vx.fe;
+                    double g0, g1, g2, g3;       // dyu, dyv, dzu, dzw of the left cell
+                    if (ARK_XSHFL(RX)) { g0 = ark_from_left(dyu); g1 = ark_from_left(dyv); g2 = ark_from_left(dzu); g3 = ark_from_left(dzw); }
+                    else { g0 = M.GB[0 * NCOL + l]; g1 = M.GB[1 * NCOL + l]; g2 = M.GB[2 * NCOL + l]; g3 = M.GB[3 * NCOL + l]; }
+                    vx = ark_visc_face(P.D.KV, u - uL, v - vL, w - wL, g0 + dyu, g1 + dyv, g2 + dzu, g3 + dzw,
+                                       uL + u, vL + v, wL + w, Tc - TL);
+                    if (!ARK_XSHFL(RX)) {
+                        M.VB[0 * NCOL + tc] = vx.t0; M.VB[1 * NCOL + tc] = vx.t1; M.VB[2 * NCOL + tc] = vx.t2; M.VB[3 * NCOL + tc] = vx.fe;
+                    }
                 }
                 {                  // face (cj-1 | cj), normal y, transverse a = x, b = z (row 1 computes it for nobody)
                     const double* L = pq - RX;
@@ -376,10 +396,13 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             ark_transport_axis<3, 1>(Tq, NCOL, tc, 1, fx.us, fx.pi, usxh, pixh, P.D.g_on[0], P.g[0], dG, work, true);
             ark_transport_axis<3, 2>(Tq, NCOL, tc, RX, fy.us, fy.pi, usyh, piyh, P.D.g_on[1], P.g[1], dG, work, false);
             if (VISC) {
-                dG[1] -= (M.VB[0 * NCOL + tc + 1] - vx.t0) + (M.VB[4 * NCOL + tc + RX] - vy.t1);
-                dG[2] -= (M.VB[1 * NCOL + tc + 1] - vx.t1) + (M.VB[5 * NCOL + tc + RX] - vy.t0);
-                dG[3] -= (M.VB[2 * NCOL + tc + 1] - vx.t2) + (M.VB[6 * NCOL + tc + RX] - vy.t2);
-                dG[4] -= (M.VB[3 * NCOL + tc + 1] - vx.fe) + (M.VB[7 * NCOL + tc + RX] - vy.fe);
+                double h0, h1, h2, h3;           // viscous flux through the high-x face = the right cell's low-x face
+                if (ARK_XSHFL(RX)) { h0 = ark_from_right(vx.t0); h1 = ark_from_right(vx.t1); h2 = ark_from_right(vx.t2); h3 = ark_from_right(vx.fe); }
+                else { h0 = M.VB[0 * NCOL + tc + 1]; h1 = M.VB[1 * NCOL + tc + 1]; h2 = M.VB[2 * NCOL + tc + 1]; h3 = M.VB[3 * NCOL + tc + 1]; }
+                dG[1] -= (h0 - vx.t0) + (M.VB[4 * NCOL + tc + RX] - vy.t1);
+                dG[2] -= (h1 - vx.t1) + (M.VB[5 * NCOL + tc + RX] - vy.t0);
+                dG[3] -= (h2 - vx.t2) + (M.VB[6 * NCOL + tc + RX] - vy.t2);
+                dG[4] -= (h3 - vx.fe) + (M.VB[7 * NCOL + tc + RX] - vy.fe);
             }
             // low z face enters with +lam*G_z and the gravity work dt g_z max(m,0); the source lam*S_i
             M.acc[0] = (Uc[0] - lam * dG[0]) + lam * Gz[0];
