@@ -84,6 +84,7 @@ struct ark_solver {
     dim3 step_grid;
     int zchunk;
     long long launches;
+    CUtensorMap tmap[2];    // 3D: tensor maps of the two padded states (TMA tile loads of the step kernel)
     double* h_pinned;       // 2 doubles, pinned, for the 16-byte D2H of compute_dt
     // optional event bracketing of the step kernel (measurement hook)
     bool timing;
@@ -93,6 +94,31 @@ struct ark_solver {
 };
 
 namespace {
+
+// Tensor map of one padded 3D state for the step kernel's TMA loads: 4-D tensor (x, y, z, field) of fp64, box =
+// (RX columns, RY rows, 1 plane, 5 fields), no swizzle, zero fill outside the array (ragged tiles).  The encoder is a
+// driver entry point fetched through the runtime, so the library does not link libcuda.
+int make_tensor_map(CUtensorMap* out, const Layout& L, double* base, int rx, int ry) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        ARK_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) return fail(ARK_ECUDA, "cuTensorMapEncodeTiled is not available%s");
+        encode = (encode_fn)fn;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)L.px, (cuuint64_t)L.py, (cuuint64_t)L.pz, (cuuint64_t)L.nf};
+    const cuuint64_t strides[3] = {(cuuint64_t)L.px * 8, (cuuint64_t)L.px * L.py * 8, (cuuint64_t)L.fstride * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)rx, (cuuint32_t)ry, 1, (cuuint32_t)L.nf};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(ARK_ECUDA, "cuTensorMapEncodeTiled failed (%s%lld)", "", (long long)r);
+    return ARK_OK;
+}
 
 int grid_for(long long n, int block, int cap = 148 * 8) {
     long long b = (n + block - 1) / block;
@@ -112,7 +138,7 @@ int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
     if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
     kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
-                                                            s->scratch, s->zchunk);
+                                                            s->scratch, s->zchunk, s->tmap[s->cur]);
     if (timed) { ARK_CUDA(cudaEventRecord(s->ev1[s->n_timed], s->stream)); s->n_timed++; }
     ARK_CUDA(cudaGetLastError());
     s->launches++;
@@ -259,6 +285,12 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     if ((long long)s->step_grid.x * s->step_grid.y * s->step_grid.z > MAX_SCRATCH) {
         delete s;
         return fail(ARK_EINVAL, "ark_create: grid too large for the rate scratch%s");
+    }
+    if (ndim == 3) {
+        for (int b = 0; b < 2; ++b) {
+            const int rc = make_tensor_map(&s->tmap[b], L, s->U[b], TX3 + 4, TY3 + 4);
+            if (rc != ARK_OK) { delete s; return rc; }
+        }
     }
     cudaError_t e = cudaMallocHost((void**)&s->h_pinned, 2 * sizeof(double));
     if (e != cudaSuccess) { delete s; return fail(ARK_ECUDA, "CUDA error: %s", cudaGetErrorString(e)); }

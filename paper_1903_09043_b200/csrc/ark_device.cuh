@@ -11,6 +11,7 @@
 #pragma once
 
 #ifndef ARK_HOST_EMU
+#include <cuda.h>           // CUtensorMap (type only; the encoder is fetched through the runtime, see ark.cu)
 #include <cuda_runtime.h>
 #define ARK_DEV __device__ __forceinline__
 #define ARK_GLOBAL __global__
@@ -111,9 +112,11 @@ ARK_DEV double ark_rsqrt(double x) {
 #endif
 }
 
-// TMA bulk copies global -> shared (cp.async.bulk, SASS UBLKCP) completing on an mbarrier: the U^n prefetch ring of
-// the 3D step kernel.  One elected lane issues whole 256-byte rows; the data never passes through registers or the
-// LSU pipe of the issuing warp.  (Host emulation: see ark_step.cuh, the copies are done synchronously per thread.)
+// TMA tile loads global -> shared (cp.async.bulk.tensor, SASS UTMALDG) completing on an mbarrier: the U^n prefetch
+// ring of the 3D step kernel.  ONE thread of the block issues ONE instruction per plane: a 4-D box (RX columns x RY rows
+// x 1 plane x 5 fields) of the padded SoA state; out-of-range columns / rows of ragged tiles are zero-filled by the TMA
+// unit.  The data never passes through registers or the LSU pipe.  (Host emulation: see ark_step.cuh, the copies are
+// done synchronously per thread.)
 #ifndef ARK_HOST_EMU
 ARK_DEV unsigned ark_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 ARK_DEV void ark_mbar_init(unsigned long long* bar, unsigned count) {
@@ -126,9 +129,9 @@ ARK_DEV void ark_mbar_fence_init() {
 ARK_DEV void ark_mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ark_smem_u32(bar)), "r"(bytes) : "memory");
 }
-ARK_DEV void ark_bulk_g2s(double* smem_dst, const double* gsrc, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(ark_smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(ark_smem_u32(bar)) : "memory");
+ARK_DEV void ark_tma_load_4d(double* smem_dst, const void* tmap, int c0, int c1, int c2, int c3, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(ark_smem_u32(smem_dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(ark_smem_u32(bar)) : "memory");
 }
 ARK_DEV void ark_mbar_wait(unsigned long long* bar, unsigned parity) {
     asm volatile(

@@ -161,11 +161,10 @@ struct ArkMarch {
     double *UR, *PB, *FB, *TB, *GB, *VB;
     const double* Ucol;
     const double* Ucol2;                 // ring rows: the edge column (row 0 or RY-1) this thread also serves
-    const double *Urow, *Urow2;          // column 0 of the own row / of the edge row (TMA bulk copies of whole rows)
-    unsigned long long* mbar;            // the row's three mbarriers (one per UR slot)
+    const void* tmap;                    // tensor map of the input state (TMA tile loads of the UR ring)
+    int tx, ty;                          // box origin in the padded array (columns, rows)
+    unsigned long long* mbar;            // the block's three mbarriers (one per UR slot)
     unsigned phase;                      // parity bit of each slot's next completion
-    int row0, row2;                      // first column index of the own row / the edge row
-    bool leader;                         // lane 0 of the row: issues the copies
     double* Ocol;
     long long pstride, fs;
     int tc, tc2, k0, k1;
@@ -179,26 +178,19 @@ struct ArkMarch {
     ark_u64 rate_max;
 };
 
-// U^n(k) of this thread's row(s) -> UR[slot].  GPU: lane 0 of the row's warp issues one 256-byte TMA bulk copy per
-// field (and the same for the edge row a ring warp serves), all completing on the warp's mbarrier of that slot.
-// Host emulation: every thread copies its own column(s) synchronously.
+// U^n(k) of the whole region -> UR[slot].  GPU: thread 0 of the block issues one TMA tile load (box RX x RY x 1 plane
+// x 5 fields, laid out in shared memory exactly as UR[slot][field][row][column]) completing on the block's mbarrier
+// of that slot.  Host emulation: every thread copies its own column(s) synchronously.
 template <bool VISC, int TX, int TY>
 ARK_DEV void ark_ring_issue(const ArkMarch<VISC, TX, TY>& M, int k, int slot, bool edge) {
     using C = ArkStepCfg<3, VISC, TX, TY>;
     constexpr int NCOL = C::NCOL;
 #ifndef ARK_HOST_EMU
-    if (M.leader) {
-        constexpr unsigned ROWB = C::RX * sizeof(double);
+    (void)edge;
+    if (threadIdx.x == 0) {
         unsigned long long* bar = M.mbar + slot;
-        ark_mbar_expect_tx(bar, (edge ? 10u : 5u) * ROWB);
-        const double* __restrict__ c = M.Urow + M.pstride * (long long)k;
-        double* d = M.UR + slot * 5 * NCOL + M.row0;
-        for (int f = 0; f < 5; ++f) ark_bulk_g2s(d + f * NCOL, c + f * M.fs, ROWB, bar);
-        if (edge) {
-            const double* __restrict__ c2 = M.Urow2 + M.pstride * (long long)k;
-            double* d2 = M.UR + slot * 5 * NCOL + M.row2;
-            for (int f = 0; f < 5; ++f) ark_bulk_g2s(d2 + f * NCOL, c2 + f * M.fs, ROWB, bar);
-        }
+        ark_mbar_expect_tx(bar, 5u * NCOL * (unsigned)sizeof(double));
+        ark_tma_load_4d(M.UR + slot * 5 * NCOL, M.tmap, M.tx, M.ty, k + ARK_NG, 0, bar);
     }
 #else
     for (int e = 0; e < (edge ? 2 : 1); ++e) {
@@ -435,7 +427,8 @@ ARK_DEV void ark_march(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
 
 template <bool VISC, int TX, int TY>
 ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
-                        const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem) {
+                        const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem,
+                        const void* tmap) {
     using C = ArkStepCfg<3, VISC, TX, TY>;
     constexpr int RX = C::RX, RY = C::RY, NCOL = C::NCOL, NP = C::NP;
     ArkMarch<VISC, TX, TY> M;
@@ -446,7 +439,7 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.GB = M.TB + 10 * NCOL;                          // [7][NCOL]: dyu,dyv,dzu,dzw,dxv,dxu,dzv (VISC)
     M.VB = M.GB + (VISC ? 7 : 0) * NCOL;              // [8][NCOL]: viscous low-face fluxes x(4), y(4) (VISC)
     ark_u64* red = (ark_u64*)(M.VB + (VISC ? 8 : 0) * NCOL);   // [32]
-    unsigned long long* mbars = red + 32;             // [RY-2][3]
+    unsigned long long* mbars = red + 32;             // [3]
 
     // thread -> column of rows 1..RY-2 (one warp per row when RX == 32)
     const int t = threadIdx.x;
@@ -475,17 +468,13 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.Ucol2 = M.Ucol + (long long)P.px * (long long)(lj2 - lj);
     M.Ocol = Uout + colbase + M.pstride * (long long)P.offz;
     M.fs = P.fstride;
-    // whole rows for the bulk copies start at region column 0 (never clamped in x: a ragged tile's row runs on into
-    // the padding / the next row, valid memory whose values nobody consumes)
-    M.Urow = M.Ucol - (li - (int)(blockIdx.x * TX - 2));
-    M.Urow2 = M.Ucol2 - (li - (int)(blockIdx.x * TX - 2));
-    M.row0 = cj * RX;
-    M.row2 = M.top ? M.row0 + RX : M.row0 - RX;
-    M.leader = ci == 0;
-    M.mbar = mbars + 3 * (cj - 1);
+    M.tmap = tmap;
+    M.tx = (int)(blockIdx.x * TX) - 2 + ARK_XOFF;
+    M.ty = (int)(blockIdx.y * TY) - 2 + ARK_NG;
+    M.mbar = mbars;
     M.phase = 0;
 #ifndef ARK_HOST_EMU
-    if (M.leader) {
+    if (t == 0) {
         for (int s3 = 0; s3 < 3; ++s3) ark_mbar_init(M.mbar + s3, 1);
         ark_mbar_fence_init();
     }
@@ -682,14 +671,23 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
     }
 }
 
+// the tensor map of the input state rides in the kernel parameter bank (3D; the 2D kernels ignore it)
+#ifndef ARK_HOST_EMU
+#define ARK_TMAP_PARAM , const __grid_constant__ CUtensorMap tmap
+#define ARK_TMAP_ARG &tmap
+#else
+#define ARK_TMAP_PARAM
+#define ARK_TMAP_ARG nullptr
+#endif
+
 template <int NDIM, bool VISC, int TX, int TY>
 ARK_GLOBAL void
 #ifndef ARK_HOST_EMU
 __launch_bounds__(ArkStepCfg<NDIM, VISC, TX, TY>::NT, 1)
 #endif
 ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict__ Uout,
-           double dt_value, const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk) {
+           double dt_value, const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk ARK_TMAP_PARAM) {
     ARK_DYN_SMEM(smem);
-    if (NDIM == 3) ark_step3d<VISC, TX, TY>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, zchunk, smem);
+    if (NDIM == 3) ark_step3d<VISC, TX, TY>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, zchunk, smem, ARK_TMAP_ARG);
     else           ark_step2d<VISC, TX, TY>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, smem);
 }
