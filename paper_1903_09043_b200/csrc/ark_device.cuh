@@ -80,10 +80,11 @@ ARK_DEV ark_u64 ark_umax(ark_u64 a, ark_u64 b) { return a > b ? a : b; }
 
 // ------------------------------------------------------------------------------------------------
 // Fast fp64 reciprocal and reciprocal square root for the step kernel: the hardware seed (MUFU.RCP64H /
-// MUFU.RSQ64H through rcp/rsqrt.approx.ftz.f64, ~2^-20 relative) followed by one third-order and one
-// second-order Newton step, no special-case branches (arguments are finite, normal and positive for every
-// valid cell; garbage lanes may produce inf/NaN that no valid cell consumes).  Relative error <= ~1 ulp,
-// against ~20 instructions plus a slow-path call for the IEEE division.
+// MUFU.RSQ64H through rcp/rsqrt.approx.ftz.f64; measured on B200: relative error 9.8e-7 / 9.1e-7) followed by ONE
+// third-order Newton step, no special-case branches (arguments are finite, normal and positive for every valid cell;
+// garbage lanes may produce inf/NaN that no valid cell consumes).  Measured maximum relative error over 2^20 random
+// arguments in [2^-20, 2^21): 1.11e-16 (rcp), 1.38e-16 (rsqrt), i.e. <= 1.25 x 2^-53 -- against ~10 fp64
+// instructions plus a slow-path call for the IEEE division.
 // ------------------------------------------------------------------------------------------------
 ARK_DEV double ark_rcp(double x) {
 #ifndef ARK_HOST_EMU
@@ -91,9 +92,7 @@ ARK_DEV double ark_rcp(double x) {
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     double e = fma(-x, y, 1.0);
     e = fma(e, e, e);
-    y = fma(y, e, y);                  // error ~ seed^3
-    e = fma(-x, y, 1.0);
-    return fma(y, e, y);
+    return fma(y, e, y);               // y (1 + e + e^2): error ~ seed^3
 #else
     return 1.0 / x;
 #endif
@@ -103,10 +102,8 @@ ARK_DEV double ark_rsqrt(double x) {
 #ifndef ARK_HOST_EMU
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x * y, y, 1.0);                    // 1 - x y^2
-    y = fma(y * e, fma(0.375, e, 0.5), y);             // y (1 + e/2 + 3 e^2/8)
-    e = fma(-x * y, y, 1.0);
-    return fma(0.5 * y, e, y);
+    const double e = fma(-x * y, y, 1.0);              // 1 - x y^2
+    return fma(y * e, fma(0.375, e, 0.5), y);          // y (1 + e/2 + 3 e^2/8): error ~ seed^3
 #else
     return 1.0 / std::sqrt(x);
 #endif
