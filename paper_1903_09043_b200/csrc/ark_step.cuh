@@ -58,7 +58,11 @@ struct ArkStepCfg {
 // sign tests on the integer pipe (the fp64 pipe is the bottleneck of this kernel): for u* >= 0 the paper's
 // upwind choice is the left cell (reading A10); -0.0 picks the right cell, whose flux is
 // multiplied by that same zero.
+#ifndef ARK_HOST_EMU
+ARK_DEV bool ark_nonneg(double x) { return __double2hiint(x) >= 0; }
+#else
 ARK_DEV bool ark_nonneg(double x) { return (int)(__double_as_longlong(x) >> 32) >= 0; }
+#endif
 ARK_DEV double ark_pos_part(double x) { return ark_nonneg(x) ? x : 0.0; }   // max(x, 0)
 ARK_DEV double ark_neg_part(double x) { return ark_nonneg(x) ? 0.0 : x; }   // min(x, 0)
 
@@ -165,7 +169,7 @@ struct ArkMarch {
     int tx, ty;                          // box origin in the padded array (columns, rows)
     unsigned long long* mbar;            // the block's three mbarriers (one per UR slot)
     unsigned phase;                      // parity bit of each slot's next completion
-    double* Ocol;
+    double* Ocur;                        // tile rows: plane q-1 of the own column in the output state
     long long pstride, fs;
     int tc, tc2, k0, k1;
     bool inU, want_rate, top;            // top: ring row RY-2 (its edge row RY-1 owns a low-y face)
@@ -368,7 +372,7 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
                 for (int f = 0; f < 5; ++f) out[f] = M.acc[f] - lam * Gz[f];
                 if (P.D.g_on[2]) out[4] += K.dt * P.g[2] * ark_neg_part(mzf);
                 if (M.inU) {
-                    double* __restrict__ c = M.Ocol + M.pstride * (long long)(q - 1);
+                    double* __restrict__ c = M.Ocur;             // plane q-1 of the own column
                     c[0] = out[0];
                     c[M.fs] = out[1];
                     c[2 * M.fs] = out[2];
@@ -408,7 +412,14 @@ ARK_DEV void ark_plane(const ArkParams& P, const ArkStepConst& K, ArkMarch<VISC,
             }
         }
     }
-    // rotate the rings
+    // rotate the rings; the output pointer follows plane q (kept in registers: recomputing it from the block and
+    // thread indices costs ~40 integer instructions per plane)
+    if (ROLE == 2) {
+        M.Ocur += M.pstride;
+#ifndef ARK_HOST_EMU
+        asm volatile("" : "+l"(M.Ocur));
+#endif
+    }
     M.zlo = zhi;
     if (VISC) { M.wm[0] = u; M.wm[1] = v; M.wm[2] = w; M.wm[3] = M.wc.T; }
     M.wc = wn;
@@ -466,7 +477,7 @@ ARK_DEV void ark_step3d(const ArkParams& P, const double* __restrict__ Uin, doub
     M.pstride = (long long)P.px * P.py;
     M.Ucol = Uin + colbase + M.pstride * (long long)P.offz;    // plane 0 of this column
     M.Ucol2 = M.Ucol + (long long)P.px * (long long)(lj2 - lj);
-    M.Ocol = Uout + colbase + M.pstride * (long long)P.offz;
+    M.Ocur = Uout + colbase + M.pstride * (long long)(P.offz + M.k0 - 2);   // plane q-1 at q = k0-1
     M.fs = P.fstride;
     M.tmap = tmap;
     M.tx = (int)(blockIdx.x * TX) - 2 + ARK_XOFF;
