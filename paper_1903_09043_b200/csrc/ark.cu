@@ -147,7 +147,10 @@ int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
 
 int launch_bc(ark_solver* s, double* U) {
     const ArkParams& P = s->P;
-    {
+    if (P.bc[0][0] == ARK_BCK_PERIODIC) {
+        const long long n = 2LL * P.ny * P.nz * P.nf;
+        ark_k_bc_x_periodic<<<grid_for(n, 256, 148 * 16), 256, 0, s->stream>>>(P, U);
+    } else {
         const long long n = 2LL * P.ny * P.nz;
         ark_k_bc<0><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
     }

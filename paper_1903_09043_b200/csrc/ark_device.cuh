@@ -312,6 +312,31 @@ ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
     }
 }
 
+// Periodic x sweep: a pure copy of two cells per (row, side, field).  The general kernel above walks the fields and
+// layers of a row end serially in one thread; every access of this sweep is a lone 32-byte sector (row ends are a
+// pitch apart), so the only lever is parallelism: one thread per (row, side, field), both layers in one 16-byte
+// access when nx is even (ghost and source pairs are then 16-byte aligned: interior cell 0 sits at an even index).
+ARK_GLOBAL void ark_k_bc_x_periodic(ArkParams P, double* __restrict__ U) {
+    const long long nrow = (long long)P.ny * P.nz;
+    const long long n = nrow * 2 * P.nf;
+    const bool vec = (P.nx & 1) == 0;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int f = (int)(s / (2 * nrow));
+        const long long rem = s - (long long)f * 2 * nrow;
+        const int side = (int)(rem / nrow);
+        const long long r = rem - (long long)side * nrow;
+        const long long base = f * P.fstride + ark_idx(P, 0, (int)(r % P.ny), (int)(r / P.ny));
+        const long long dst = side == 0 ? base - ARK_NG : base + P.nx;            // ghosts -2,-1 | nx,nx+1
+        const long long src = side == 0 ? base + P.nx - ARK_NG : base;            // cells nx-2,nx-1 | 0,1
+#ifndef ARK_HOST_EMU
+        if (vec) { *reinterpret_cast<double2*>(U + dst) = *reinterpret_cast<const double2*>(U + src); continue; }
+#endif
+        const double a = U[src], b = U[src + 1];
+        U[dst] = a; U[dst + 1] = b;
+        (void)vec;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // CFL rate of one cell (reading A4):
 //   rate = sum_d (|u_d| + c)/h + 2 ndim max(4 mu/3, (gamma-1) kappa) / (rho h^2)

@@ -71,7 +71,12 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
     grid.z = P.ndim == 3 ? (nz + zchunk - 1) / zchunk : 1;
     const bool visc = mu > 0.0 || kappa > 0.0;
     for (int s = 0; s < nsteps; ++s) {
-        bc<0>(P, cur, 2LL * ny * nz);
+        if (P.bc[0][0] == ARK_BCK_PERIODIC) {     // mirrors launch_bc in csrc/ark.cu
+            emu_dim3 gp; gp.x = (unsigned)((2LL * ny * nz * P.nf + 63) / 64);
+            ark_emu_launch(gp, 64, 0, [&] { ark_k_bc_x_periodic(P, cur); });
+        } else {
+            bc<0>(P, cur, 2LL * ny * nz);
+        }
         bc<1>(P, cur, 2LL * (nx + 4) * nz);
         if (P.ndim == 3) bc<2>(P, cur, 2LL * (nx + 4) * (ny + 4));
         if (s == 0 && padded_out) {
