@@ -5,24 +5,24 @@
 // state U~ live in registers / shared memory only.
 //
 // Decomposition ("2.5-D marching"): a block owns a TX x TY tile of (x,y) columns plus a 2-cell halo
-// (region RX x RY = (TX+4) x (TY+4), one thread per column) and marches along z over a chunk of planes.
-// The product build uses TX = 28, so RX = 32: ONE WARP PER REGION ROW.  Every role in the kernel depends on
-// the ROW only (halo row / ring row / output row), i.e. is warp-uniform: halo warps skip whole phases, no
-// lane is predicated off inside a phase (the 4 halo lanes of a row compute values nobody consumes), and every
-// global access of a warp is one contiguous 256-byte row segment.  Only the final stores and the CFL rate
-// carry a per-lane predicate.
+// (region RX x RY = (TX+4) x (TY+4)) and marches along z over a chunk of planes.  The product build uses
+// TX = 28, so RX = 32: ONE WARP PER REGION ROW 1..RY-2 (the two edge rows 0 and RY-1 only need primitives and are
+// the second column of the ring-row threads).  Every role in the kernel depends on the ROW only (ring row / tile row),
+// i.e. is warp-uniform and a compile-time parameter of the plane loop: no lane is predicated off inside a phase (the
+// 4 halo lanes of a row compute values nobody consumes); only the final stores and the CFL rate carry a per-lane
+// predicate.
 //
-// What persists from plane to plane lives in shared memory rings owned by the column's thread --
-//   UR  U^n of planes q, q+1, q+2   (filled by 8-byte cp.async two planes ahead: the HBM prefetch costs no
-//                                    registers and no instructions on the critical path)
-//   PB  primitives of planes q-1, q, q+1 (x/y neighbours read them; the own column's z neighbours too)
-//   TB  U~ of planes q-1, q
-// -- so the register pipeline along z is only the running update acc[5], the low z face and four velocity
-// differences, and nothing has to be rotated through registers at the end of an iteration.
+// What persists from plane to plane --
+//   UR  U^n of planes q, q+1, q+2 in shared memory, filled two planes ahead by ONE TMA tensor tile load per block
+//       and plane (cp.async.bulk.tensor, 4-D box RX x RY x 1 x 5 fields, completion on an mbarrier): the HBM
+//       prefetch costs no registers, no LSU wavefronts and one instruction of one thread
+//   PB  primitives of planes q, q+1 in shared memory (the x/y neighbours read them)
+//   TB  U~ of planes q-1, q in shared memory
+//   registers: the own column's primitives of plane q and u,v,w,T of plane q-1, the running update acc[5], the low
+//   z face and four velocity differences.
 //
-// Per plane q one iteration does (3 block barriers):
+// Per plane q one iteration does (2 block barriers):
 //   S1  primitives of plane q+1 (own column, from the UR ring)          -> PB
-//   --- barrier A
 //   S2  acoustic faces x-, y- of plane q (neighbours from PB), z face (q|q+1) from the own column   -> FB
 //       cell-centred velocity differences of plane q                                               -> GB
 //   --- barrier B
@@ -32,6 +32,8 @@
 //   S4  transport fluxes (upwind on u*) of the in-plane faces of plane q and of the
 //       z face (q-1|q); completes and stores U^{n+1}(q-1); folds the CFL rate of the new state into a
 //       per-block maximum (integer max on the bit patterns, NaN-propagating).
+// What only the x neighbour consumes (high-x acoustic face, the left cell's differences, the high-x viscous flux) is
+// exchanged by warp shuffle and never touches shared memory.
 #pragma once
 #include "ark_device.cuh"
 
