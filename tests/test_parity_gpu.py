@@ -322,3 +322,18 @@ def test_full_size_sampled_parity(B, cfg):
             g = out[f][k0:k0 + W, j0:j0 + W, i0:i0 + W].cpu().numpy()
             scale = np.abs(r).max()
             assert np.abs(r - g).max() <= 1e-12 * scale, (cfg, (k0, j0, i0), f, np.abs(r - g).max(), scale)
+
+
+def test_results_are_bitwise_reproducible(B):
+    """compute-sanitizer is closed on this pool, so shared-memory hazards are hunted the other way: a data race in the
+    step kernel (rings, barriers, shuffles, TMA completion) shows up as run-to-run differences.  Five runs of a ragged,
+    viscous, walled 3D case and of a 2D case must agree bit for bit (and with the oracle to 1e-12, above)."""
+    for name in ("3d_walls_viscous", "3d_all_walls_oblique", "2d_walls_gravity_viscous"):
+        prm, U = RANDOM[name]()
+        _, dts = O.run(prm, U, 6, cfl=0.4)
+        first = gpu_run(B, prm, U, dts)
+        for _ in range(4):
+            again = gpu_run(B, prm, U, dts)
+            for f in range(5):
+                if first[f] is not None:
+                    assert np.array_equal(first[f], again[f]), (name, f)
