@@ -11,7 +11,7 @@
 // Build:  g++ -O2 -ffp-contract=off -fno-fast-math -shared -fPIC   (oracle/build.py)
 // No blocking, fusion or reordering beyond what the paper's algorithm states:
 // the step is the literal sequence
-//   1. ghost fill            (reading A9)
+//   1. ghost fill            (readings A9, A22)
 //   2. primitives
 //   3. acoustic face values
 //   4. acoustic update -> U~ (reading A3)
@@ -42,7 +42,7 @@ namespace {
 constexpr int NG = 2;          // ghost layers per side (reading A9)
 constexpr double K_IMP = 1.1;  // a = K*max(rho_L c_L, rho_R c_R)  (reading A2)
 
-enum { BC_PERIODIC = 0, BC_REFLECTING = 1, BC_FIXED_T = 2 };
+enum { BC_PERIODIC = 0, BC_REFLECTING = 1, BC_FIXED_T = 2, BC_FLUX = 3 };
 
 struct Cfg {
     int n[3];        // interior cells per axis; n[2]==1 -> 2D (reading A18)
@@ -54,7 +54,7 @@ struct Cfg {
     double kappa;    // thermal conductivity
     int theta;       // 0: theta == 1 ; 1: eq. (13)
     int bc[3][2];    // [axis][lo,hi]
-    double bcv[3][2];// wall temperature for BC_FIXED_T
+    double bcv[3][2];// wall temperature for BC_FIXED_T; heat flux entering the domain for BC_FLUX
 };
 
 struct Grid {
@@ -171,6 +171,11 @@ void fill_ghosts(const Cfg& cfg, const Grid& G, State& U) {
                     if (type == BC_REFLECTING) {
                         for (int e = 0; e < 3; ++e) ug[e] = (e == d) ? -ws.u[e] : ws.u[e];
                         Tg = ws.T;
+                    } else if (type == BC_FLUX) {                   // imposed temperature flux, PAPER.md:435 (reading A22)
+                        // reflecting velocity; the conductive flux kappa (T_ghost - T_mirror)/((2l-1) h) through
+                        // the wall equals the prescribed flux F entering the domain
+                        for (int e = 0; e < 3; ++e) ug[e] = (e == d) ? -ws.u[e] : ws.u[e];
+                        Tg = ws.T + (2 * l - 1) * cfg.bcv[d][side] * cfg.h / cfg.kappa;
                     } else {                                        // BC_FIXED_T no-slip wall
                         for (int e = 0; e < 3; ++e) ug[e] = -ws.u[e];
                         Tg = 2.0 * cfg.bcv[d][side] - ws.T;

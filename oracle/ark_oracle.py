@@ -10,7 +10,7 @@ import numpy as np
 
 from . import build as _build
 
-BC_PERIODIC, BC_REFLECTING, BC_FIXED_T = 0, 1, 2
+BC_PERIODIC, BC_REFLECTING, BC_FIXED_T, BC_FLUX = 0, 1, 2, 3
 
 _lib = None
 _dp = C.POINTER(C.c_double)

@@ -588,3 +588,57 @@ def test_cfl_closed_form_and_stability_margin():
     S, _ = O.run(prm3, U3, 60, cfl=0.4)
     rho_, u_, v_, w_, p_ = prim(prm3, S)
     assert rho_.min() > 0 and p_.min() > 0
+
+
+# ----------------------------------------------------------------------------------------------- imposed-flux wall (A22)
+FLX = I.BC_FLUX
+
+
+def test_flux_wall_energy_budget_closed_form():
+    """PAPER.md:435 "we impose the temperature flux on the bottom boundary" (reading A22).  With u*_wall = 0 the only
+    energy that crosses a flux wall is the conductive flux kappa (T_ghost - T_0)/h = F, so per step
+    Delta sum(E + rho Phi) = dt * (face cells) * (F_lo + F_hi) / h exactly, and mass is conserved (mu = 0: no wall stress
+    work; the state is a random one, not an equilibrium)."""
+    for dim in (2, 3):
+        Flo, Fhi = 0.037, -0.011
+        if dim == 2:
+            prm, U = I.random_state(12, 16, 1, 21, g=(0, -1.0, 0), mu=0.0, kappa=5e-2,
+                                    bc_type=((PER, PER), (FLX, FLX), (0, 0)), bc_value=((0, 0), (Flo, Fhi), (0, 0)))
+            nface = prm["nx"]
+        else:
+            prm, U = I.random_state(6, 7, 10, 22, g=(0, 0, -1.0), mu=0.0, kappa=5e-2,
+                                    bc_type=((PER, PER), (PER, PER), (FLX, FLX)), bc_value=((0, 0), (0, 0), (Flo, Fhi)))
+            nface = prm["nx"] * prm["ny"]
+        shape = (prm["nz"], prm["ny"], prm["nx"])
+        S = [a if a is not None else np.zeros_like(U[0]) for a in U]
+        for _ in range(5):
+            t0 = _totals(prm, [a.reshape(-1) for a in S], shape)
+            S, dts = O.run(prm, S, 1, cfl=0.4)
+            t1 = _totals(prm, S, shape)
+            expect = dts[0] * nface * (Flo + Fhi) / prm["dx"]
+            assert abs((t1[4] - t0[4]) - expect) < 1e-12 * abs(t0[4]), (dim, t1[4] - t0[4], expect)
+            assert abs(t1[0] - t0[0]) < 1e-13 * t0[0]
+
+
+def test_flux_wall_with_zero_flux_is_the_reflecting_wall():
+    prm, U = I.random_state(14, 12, 1, 23, g=(0, -1.0, 0), mu=1e-3, kappa=2e-3, bc_type=((PER, PER), (FLX, FLX), (0, 0)))
+    ref = dict(prm, bc_type=((PER, PER), (REF, REF), (0, 0)))
+    A, _ = O.run(prm, U, 4, cfl=0.4)
+    B, _ = O.run(ref, U, 4, cfl=0.4)
+    for f in (0, 1, 2, 4):
+        assert np.array_equal(A[f], B[f]), f
+
+
+def test_flux_wall_feeding_the_conductive_flux_keeps_the_polytrope_at_rest():
+    """The paper's 2D Rayleigh-Benard walls: temperature flux imposed at the bottom, here equal to the
+    conductive flux kappa*beta of the linear profile, fixed temperature at the top: the layer built with (14) is a
+    steady state of the scheme (the wall face carries exactly the flux every interior face carries)."""
+    prm, U = I.config3_rb2d(nx=8, ny=48, amp=0.0)
+    beta = 1.0 / 2.3
+    bt = ((PER, PER), (FLX, FIX), (0, 0))
+    bv = ((0, 0), (prm["kappa"] * beta, prm["bc_value"][1][1]), (0, 0))
+    prm = dict(prm, bc_type=bt, bc_value=bv)
+    S, _ = O.run(prm, U, 300, cfl=0.4)
+    # a flux wall reflects the velocity (free slip): the rest state must survive it as it does the no-slip wall
+    assert max(np.abs(S[1] / S[0]).max(), np.abs(S[2] / S[0]).max()) < 1e-12
+    assert np.max(np.abs(S[4] - U[4].reshape(-1)) / U[4].reshape(-1)) < 1e-12
