@@ -38,12 +38,14 @@ typedef struct ark_solver ark_solver; /* opaque, owned by the library */
 enum { ARK_OK = 0, ARK_EINVAL = -1, ARK_ENOMEM = -2, ARK_ECUDA = -3, ARK_ENONFINITE = -4 };
 
 /* Boundary kinds (A9; PAPER.md:295 ghost zones, :378 reflecting + hydrostatic extrapolation,
- * :457 fixed temperature).  Periodic must be set on both sides of an axis. */
-enum { ARK_BC_PERIODIC = 0, ARK_BC_REFLECTING = 1, ARK_BC_FIXED_T_WALL = 2 };
+ * :457 fixed temperature, :435 imposed temperature flux).  Periodic must be set on both sides of an axis. */
+enum { ARK_BC_PERIODIC = 0, ARK_BC_REFLECTING = 1, ARK_BC_FIXED_T_WALL = 2, ARK_BC_FLUX_WALL = 3 };
 
 typedef struct {
     int type[3][2];     /* [axis x,y,z][lo,hi] */
-    double value[3][2]; /* wall temperature for ARK_BC_FIXED_T_WALL (T = p/rho, A8); ignored otherwise */
+    double value[3][2]; /* ARK_BC_FIXED_T_WALL: wall temperature (T = p/rho, A8).  ARK_BC_FLUX_WALL (PAPER.md:435,
+                           A22): conductive heat flux ENTERING the domain through this wall, any sign; the velocity
+                           is reflected as at a reflecting wall; needs kappa > 0.  Ignored otherwise. */
 } ark_bc;
 
 /* Bytes of device workspace ark_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libark_b200.so")
 
 ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
-BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL = 0, 1, 2
+BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
            "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_debug_get_padded",

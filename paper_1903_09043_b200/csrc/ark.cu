@@ -228,8 +228,10 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     for (int d = 0; d < ndim; ++d) {
         for (int sd = 0; sd < 2; ++sd) {
             const int t = bc->type[d][sd];
-            if (t != ARK_BC_PERIODIC && t != ARK_BC_REFLECTING && t != ARK_BC_FIXED_T_WALL)
+            if (t != ARK_BC_PERIODIC && t != ARK_BC_REFLECTING && t != ARK_BC_FIXED_T_WALL && t != ARK_BC_FLUX_WALL)
                 return fail(ARK_EINVAL, "ark_create: unknown boundary kind%s");
+            if (t == ARK_BC_FLUX_WALL && !(kappa > 0.0))
+                return fail(ARK_EINVAL, "ark_create: an imposed-flux wall needs kappa > 0%s");
             if (t == ARK_BC_FIXED_T_WALL && !(bc->value[d][sd] > 0.0))
                 return fail(ARK_EINVAL, "ark_create: fixed-T wall needs a positive temperature%s");
         }

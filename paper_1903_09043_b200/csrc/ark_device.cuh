@@ -26,7 +26,7 @@
 #define ARK_NG 2             // ghost layers (A9)
 #define ARK_XOFF 4           // x index of interior cell 0 inside a padded row (>= ARK_NG)
 
-enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2 };
+enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2, ARK_BCK_FLUX = 3 };
 
 // Coefficients of the dissipative face flux (see ark_visc_face in ark_step.cuh).
 struct ArkViscCoef { double cn, ct, c43, c23t, kh; };
@@ -250,6 +250,7 @@ ARK_GLOBAL void ark_k_unpack_padded(ArkParams P, const double* __restrict__ U, d
 // (transverse position, side); it writes ghost layers 1 then 2 (layer 2 chains eq. (14) from layer 1).
 //   periodic: copy.   reflecting wall: u_n -> -u_n, T_g = T_src.
 //   fixed-T no-slip wall: u -> -u (all components), T_g = 2 T_w - T_src.
+//   imposed-flux wall (A22): u_n -> -u_n, T_g = T_src + (2l-1) F h / kappa (F = heat flux entering).
 //   rho_g from the discrete hydrostatic relation (14), PAPER.md:237:
 //       p_g - p_prev = 1/2 (rho_prev + rho_g) delta,  delta = Phi_prev - Phi_g = -+ g_d h,  p_g = rho_g T_g.
 // ------------------------------------------------------------------------------------------------
@@ -296,6 +297,9 @@ ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
             if (type == ARK_BCK_REFLECTING) {
                 ug[AXIS] = -ug[AXIS];
                 Tg = ws.T;
+            } else if (type == ARK_BCK_FLUX) {
+                ug[AXIS] = -ug[AXIS];
+                Tg = ws.T + (2 * l - 1) * P.bcv[AXIS][side] * P.h / P.kappa;
             } else {
                 ug[0] = -ug[0]; ug[1] = -ug[1]; ug[2] = -ug[2];
                 Tg = 2.0 * P.bcv[AXIS][side] - ws.T;

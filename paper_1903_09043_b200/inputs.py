@@ -17,7 +17,7 @@ import math
 
 import numpy as np
 
-BC_PERIODIC, BC_REFLECTING, BC_FIXED_T = 0, 1, 2
+BC_PERIODIC, BC_REFLECTING, BC_FIXED_T, BC_FLUX = 0, 1, 2, 3
 
 
 # --------------------------------------------------------------------------- random numbers
@@ -222,9 +222,10 @@ def config3_rb2d(nx=1024, ny=512, seed=1003, amp=1e-4, theta=1, device=None):
     return prm, [rho, zero, zero.clone() if device is not None else zero.copy(), None, E]
 
 
-def _convection3d(n, nz, m, chi, mu, kappa, wall, amp, seed, theta, device, box=None):
+def _convection3d(n, nz, m, chi, mu, kappa, wall, amp, seed, theta, device, box=None, heat=0.0):
     """3D polytropic layer under g=(0,0,-1), periodic x/y, `wall` in z, velocity noise amp*(2U-1) per
-    component.  box = ((k0,k1),(j0,j1),(i0,i1)) returns only that sub-box of the state (params stay global)."""
+    component.  box = ((k0,k1),(j0,j1),(i0,i1)) returns only that sub-box of the state (params stay global).
+    heat > 0: the bottom wall becomes an imposed-flux wall feeding heat x (conductive flux kappa*beta)."""
     h = 1.0 / nz
     gamma = 5.0 / 3.0
     beta = 1.0 / (m + 1.0)
@@ -237,9 +238,10 @@ def _convection3d(n, nz, m, chi, mu, kappa, wall, amp, seed, theta, device, box=
     p = _full(_col((rho_c * Tc)[k0:k1], 2, device), bx, by, bz, device)
     vel = [amp * _noise(seed, n, n, nz, 3, c, device, box) for c in range(3)]
     E = _energy(gamma, rho, vel[0], vel[1], vel[2], p)
+    bottom, vbot = (BC_FLUX, heat * kappa * beta) if heat > 0.0 else (wall, T_bot)
     prm = make_params(n, n, nz, h, gamma, g=(0.0, 0.0, -1.0), mu=mu, kappa=kappa, theta=theta,
-                      bc_type=((BC_PERIODIC, BC_PERIODIC), (BC_PERIODIC, BC_PERIODIC), (wall, wall)),
-                      bc_value=((0, 0), (0, 0), (T_bot, T_top)))
+                      bc_type=((BC_PERIODIC, BC_PERIODIC), (BC_PERIODIC, BC_PERIODIC), (bottom, wall)),
+                      bc_value=((0, 0), (0, 0), (vbot, T_top)))
     return prm, [rho, rho * vel[0], rho * vel[1], rho * vel[2], E]
 
 
@@ -255,10 +257,11 @@ def config4_rb3d(n=256, seed=1004, amp=1e-3, theta=1, device=None, box=None):
     return _convection3d(n, n, m, chi, mu, kappa, BC_FIXED_T, amp, seed, theta, device, box)
 
 
-def config5_convection3d(n=512, seed=1005, amp=1e-2, theta=1, device=None, box=None):
-    """BASELINE config 5: steep polytrope (m=1, chi=100), mu=1e-4, kappa=2.5e-4, reflecting (insulating) z walls,
-    velocity noise 1e-2 (the imposed-flux bottom wall is a NEXT item; it does not change the work per cell)."""
-    return _convection3d(n, n, 1.0, 100.0, 1.0e-4, 2.5e-4, BC_REFLECTING, amp, seed, theta, device, box)
+def config5_convection3d(n=512, seed=1005, amp=1e-2, theta=1, device=None, box=None, heat=10.0):
+    """BASELINE config 5: steep polytrope (m=1, chi=100), mu=1e-4, kappa=2.5e-4, heated from below at `heat` = 10 x the
+    conductive flux kappa*beta through an imposed-flux bottom wall (reading A22), reflecting (insulating)
+    top wall, velocity noise 1e-2.  heat=0 gives reflecting walls on both sides."""
+    return _convection3d(n, n, 1.0, 100.0, 1.0e-4, 2.5e-4, BC_REFLECTING, amp, seed, theta, device, box, heat=heat)
 
 
 # --------------------------------------------------------------------------- extra test problems

@@ -33,6 +33,10 @@ CASES = {
                                                        bc_value=((0, 0), (1.5, 0), (0, 0))),
     "2d_gravity_x_walls_x": lambda: I.random_state(13, 8, 1, 14, g=(-0.7, 0.3, 0),
                                                    bc_type=((REF, REF), (REF, REF), (0, 0))),
+    "2d_flux_wall": lambda: I.random_state(15, 10, 1, 24, mu=1e-3, kappa=5e-2, g=(0, -1.0, 0),
+                                           bc_type=((PER, PER), (I.BC_FLUX, FIX), (0, 0)), bc_value=((0, 0), (0.03, 1.5), (0, 0))),
+    "3d_flux_wall": lambda: I.random_state(9, 8, 9, 25, mu=1e-3, kappa=5e-2, g=(0, 0, -1.0),
+                                           bc_type=((PER, PER), (PER, PER), (I.BC_FLUX, REF)), bc_value=((0, 0), (0, 0), (0.03, 0))),
     "3d_periodic_inviscid": lambda: I.random_state(12, 9, 7, 5),
     "3d_walls_gravity_viscous": lambda: I.random_state(12, 9, 10, 6, mu=2e-3, kappa=3e-3, g=(0, 0, -1.0),
                                                        bc_type=((PER, PER), (PER, PER), (FIX, REF)),

@@ -50,7 +50,10 @@ def test_columns_satisfy_discrete_hydrostatic_relation():
     assert np.abs(lhs - rhs).max() < 1e-15
     prm, U = I.config5_convection3d(16)
     assert U[0].max() / U[0].min() > 15          # steep stratification (chi = 100 wall to wall; cell centres see less)
-    assert prm["bc_type"][2] == (I.BC_REFLECTING, I.BC_REFLECTING) and prm["mu"] == 1e-4
+    # heated from below at 10 x the conductive flux kappa*beta (beta = 1/(m+1) = 0.5), insulating top
+    assert prm["bc_type"][2] == (I.BC_FLUX, I.BC_REFLECTING) and prm["mu"] == 1e-4
+    assert abs(prm["bc_value"][2][0] - 10 * 2.5e-4 * 0.5) < 1e-15
+    assert I.config5_convection3d(16, heat=0.0)[0]["bc_type"][2] == (I.BC_REFLECTING, I.BC_REFLECTING)
     prm, U = I.config4_rb3d(8)
     assert abs(prm["mu"] - 7.473e-4) < 2e-6 and abs(prm["kappa"] - 1.8683e-3) < 5e-6
     prm, U = I.config3_rb2d(16, 8)

@@ -115,6 +115,10 @@ RANDOM = {
                                                bc_type=((PER, PER), (PER, PER), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))),
     "3d_all_walls_oblique": lambda: I.random_state(33, 10, 18, 7, mu=1e-3, kappa=0.0, g=(0.2, -0.3, -1.0),
                                                    bc_type=((REF, FIX), (FIX, REF), (REF, REF)), bc_value=((0, 2.5), (3.5, 0), (0, 0))),
+    "3d_flux_wall_heated": lambda: I.random_state(41, 23, 30, 26, mu=1e-3, kappa=5e-2, g=(0, 0, -1.0),
+                                                  bc_type=((PER, PER), (PER, PER), (I.BC_FLUX, REF)), bc_value=((0, 0), (0, 0), (0.03, 0))),
+    "2d_flux_wall_fixed_T_top": lambda: I.random_state(50, 31, 1, 27, mu=1e-3, kappa=5e-2, g=(0, -1.0, 0),
+                                                       bc_type=((PER, PER), (I.BC_FLUX, FIX), (0, 0)), bc_value=((0, 0), (0.03, 2.5), (0, 0))),
     "3d_minimum_size": lambda: I.random_state(4, 4, 4, 8, mu=1e-3, kappa=1e-3),
     "2d_minimum_size": lambda: I.random_state(4, 4, 1, 9),
 }
@@ -136,7 +140,7 @@ def test_hydrostatic_atmosphere_stays_at_rest(B):
     config-5 polytrope with mu = kappa = 0 (with conduction and INSULATING walls that column is hydrostatic but not
     in thermal equilibrium: its wall cells heat up and drive a flow, in the oracle too, so it is not a rest state;
     n = 64 keeps T_top > g h / 2 as reading A9 requires)."""
-    c5, U5 = I.config5_convection3d(64, amp=0.0)
+    c5, U5 = I.config5_convection3d(64, amp=0.0, heat=0.0)
     cases = [I.config1_atmosphere(128, amp=0.0), I.config1_atmosphere(128, amp=0.0, theta=0),
              I.config3_rb2d(64, 96, amp=0.0), I.config4_rb3d(40, amp=0.0), (dict(c5, mu=0.0, kappa=0.0), U5)]
     for prm, U in cases:
@@ -170,7 +174,7 @@ def test_uniform_state_is_bit_exact(B):
 
 
 def test_ghost_fill_matches_oracle(B):
-    for name in ("2d_walls_gravity_viscous", "3d_all_walls_oblique", "3d_periodic", "2d_gravity_x"):
+    for name in ("2d_walls_gravity_viscous", "3d_all_walls_oblique", "3d_periodic", "2d_gravity_x", "3d_flux_wall_heated"):
         prm, U = RANDOM[name]()
         ref = O.fill_ghosts(prm, U)
         s = B.Solver(prm)
@@ -310,10 +314,8 @@ def test_full_size_sampled_parity(B, cfg):
             full = U[f].reshape(n, n, n)
             blk = full[ka:kb][:, torch.as_tensor(jj, device="cuda")][:, :, torch.as_tensor(ii, device="cuda")]
             sub.append(blk.cpu().numpy())
-        wall = prm["bc_type"][2][0]
-        bt = ((PER, PER), (PER, PER), (wall if lo_wall else REF, wall if hi_wall else REF))
-        if not lo_wall and not hi_wall:
-            bt = ((PER, PER), (PER, PER), (REF, REF))
+        wlo, whi = prm["bc_type"][2]
+        bt = ((PER, PER), (PER, PER), (wlo if lo_wall else REF, whi if hi_wall else REF))
         prm_b = dict(prm, nx=W + 4, ny=W + 4, nz=kb - ka, bc_type=bt)
         ref, _ = O.run(prm_b, sub, 1, dts=[dt])
         zs = slice(0 if lo_wall else 2, (kb - ka) if hi_wall else (kb - ka - 2))
