@@ -84,7 +84,9 @@ int ark_step(ark_solver*, double dt);
 
 /* Convenience: nsteps x { dt = cfl / max rate ; step(dt) } with the time step kept on the device
  * (no host round trip per step).  If dts_out (HOST, nsteps doubles) is not NULL the step sizes are
- * copied there; the call then synchronises.  Returns ARK_ENONFINITE if a rate was not finite. */
+ * copied there; the call then synchronises.  Returns ARK_ENONFINITE if a rate was not finite.
+ * After the first step, pairs of steps are replayed from a CUDA graph captured on a stream of the library's own
+ * (ordered with the caller's stream through events): the small 2D configurations are launch-latency-bound. */
 int ark_run(ark_solver*, int nsteps, double cfl, double* dts_out);
 
 /* Ghost fill only, then copy the PADDED current state ((nx+4)*(ny+4)*(nz+4 or 1) per field, x fastest)

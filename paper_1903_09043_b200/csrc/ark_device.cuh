@@ -395,9 +395,10 @@ ARK_GLOBAL void ark_k_cfl_pass1(ArkParams P, const double* __restrict__ U, doubl
 }
 
 // pass 2: single block over the per-block values; result[0] = max rate,
-// result[1] = dt = cfl / max rate (used by the device-side time loop of ark_run).
+// result[1] = dt = cfl / max rate (used by the device-side time loop of ark_run).  With dt_log the step size is also
+// appended at dt_log[*log_count] (a device-side counter, so that the launch can be replayed from a CUDA graph).
 ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, double cfl, double* __restrict__ result,
-                                double* __restrict__ dt_log, int step_index) {
+                                double* __restrict__ dt_log, int* __restrict__ log_count) {
     ARK_SHARED double red[32];
     double m = -1.0;
     for (int s = threadIdx.x; s < nvals; s += blockDim.x) m = ark_nanmax(m, scratch[s]);
@@ -405,6 +406,6 @@ ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, d
     if (threadIdx.x == 0) {
         result[0] = m;
         result[1] = cfl / m;
-        if (dt_log) dt_log[step_index] = cfl / m;
+        if (dt_log) { const int i = *log_count; dt_log[i] = cfl / m; *log_count = i + 1; }
     }
 }

@@ -60,7 +60,7 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
         emu_dim3 gg; gg.x = 3;
         ark_emu_launch(gg, 64, 0, [&] { ark_k_cfl_pass1(P, A.data(), scratch.data()); });
         emu_dim3 one;
-        ark_emu_launch(one, 64, 0, [&] { ark_k_cfl_pass2(scratch.data(), 3, 1.0, result.data(), nullptr, 0); });
+        ark_emu_launch(one, 64, 0, [&] { ark_k_cfl_pass2(scratch.data(), 3, 1.0, result.data(), nullptr, nullptr); });
         *rate0_out = result[0];
     }
     double* cur = A.data();
@@ -92,7 +92,7 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
         if (rates_out) {
             emu_dim3 one;
             const int nv = (int)(grid.x * grid.y * grid.z);
-            ark_emu_launch(one, 64, 0, [&] { ark_k_cfl_pass2(scratch.data(), nv, 1.0, result.data(), nullptr, 0); });
+            ark_emu_launch(one, 64, 0, [&] { ark_k_cfl_pass2(scratch.data(), nv, 1.0, result.data(), nullptr, nullptr); });
             rates_out[s] = result[0];
         }
     }

@@ -202,13 +202,14 @@ def test_compute_dt_and_run_match_oracle(B):
         s.set_state(to_dev(U))
         dt0 = s.compute_dt(0.4)
         assert abs(dt0 - O.compute_dt(prm, U, 0.4)) <= 1e-13 * dt0          # standalone two-pass reduction
-        ref, dts = O.run(prm, U, 6, cfl=0.4)
+        ref, dts = O.run(prm, U, 15, cfl=0.4)
         got_dts = []
         for i in range(3):                                                   # host loop: compute_dt + step
             dt = s.compute_dt(0.4)                                           # steps 2,3 use the fused epilogue's rates
             got_dts.append(dt)
             s.step(dt)
-        got_dts += s.run(3, 0.4, want_dts=True)                              # device-side loop
+        got_dts += s.run(3, 0.4, want_dts=True)                              # device-side loop, plain launches
+        got_dts += s.run(9, 0.4, want_dts=True)                              # 1 plain step + 4 replays of the 2-step CUDA graph
         out = to_np(s.get_state())
         s.close()
         assert np.abs(np.array(got_dts) - dts).max() <= 1e-12 * dts.max(), (got_dts, dts)
