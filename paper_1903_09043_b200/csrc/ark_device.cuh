@@ -167,15 +167,18 @@ ARK_DEV ArkPrim ark_prim(const ArkParams& P, double rho, double mx, double my, d
 
 // The same with ark_rcp / ark_rsqrt (step kernel only; the ghost fill keeps the IEEE version above).
 ARK_DEV ArkPrim ark_prim_fast(const ArkParams& P, double rho, double mx, double my, double mz, double E) {
+    // arranged for a short dependency chain: |m|^2 and gamma (gamma-1) rho do not wait for the reciprocal
     ArkPrim q;
+    const double hm2 = 0.5 * (mx * mx + my * my + mz * mz);
+    const double ggr = (P.gamma * P.gm1) * rho;
     const double rinv = ark_rcp(rho);
     q.rho = rho;
     q.u = mx * rinv;
     q.v = my * rinv;
     q.w = mz * rinv;
-    const double ke = 0.5 * (mx * q.u + my * q.v + mz * q.w);
-    q.p = P.gm1 * (E - ke);
-    const double gpr = P.gamma * q.p * rho;        // (rho c)^2
+    const double ei = E - hm2 * rinv;              // rho e
+    q.p = P.gm1 * ei;
+    const double gpr = ggr * ei;                   // (rho c)^2 = gamma p rho
     q.irc = ark_rsqrt(gpr);
     q.rc = gpr * q.irc;
     q.T = q.p * rinv;

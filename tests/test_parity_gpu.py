@@ -119,6 +119,8 @@ RANDOM = {
                                                   bc_type=((PER, PER), (PER, PER), (I.BC_FLUX, REF)), bc_value=((0, 0), (0, 0), (0.03, 0))),
     "2d_flux_wall_fixed_T_top": lambda: I.random_state(50, 31, 1, 27, mu=1e-3, kappa=5e-2, g=(0, -1.0, 0),
                                                        bc_type=((PER, PER), (I.BC_FLUX, FIX), (0, 0)), bc_value=((0, 0), (0.03, 2.5), (0, 0))),
+    "3d_conduction_only": lambda: I.random_state(30, 17, 22, 28, mu=0.0, kappa=4e-3, g=(0, 0, -0.5),
+                                                 bc_type=((PER, PER), (REF, REF), (FIX, FIX)), bc_value=((0, 0), (0, 0), (2.5, 3.5))),
     "3d_minimum_size": lambda: I.random_state(4, 4, 4, 8, mu=1e-3, kappa=1e-3),
     "2d_minimum_size": lambda: I.random_state(4, 4, 1, 9),
 }
