@@ -53,7 +53,7 @@ def build_workload(name, device=None, sample=False):
 FP64_INSTR_PER_CLK_SM, N_SM, SM_MAX_MHZ = 64, 148, 1965.0
 # fp64 thread-instructions per cell update of the step kernel (halo recomputation included), from the committed ncu
 # capture of each kernel variant (profiles/): sum of DADD+DMUL+DFMA+DSETP warp instructions x 32 / cells.
-FP64_INSTR_PER_CELL = {"config5_512": 427.7, "config4_256": 456.6}
+FP64_INSTR_PER_CELL = {"config5_512": 430.6, "config4_256": 459.7}
 # dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed `ncu --set full` capture
 DRAM_TRAFFIC_BYTES = {"config5_512": 11400.4e6, "config4_256": 1423.8e6}
 
