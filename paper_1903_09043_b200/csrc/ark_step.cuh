@@ -696,7 +696,7 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
 template <int NDIM, bool VISC, int TX, int TY>
 ARK_GLOBAL void
 #ifndef ARK_HOST_EMU
-__launch_bounds__(ArkStepCfg<NDIM, VISC, TX, TY>::NT, 1)
+__launch_bounds__(ArkStepCfg<NDIM, VISC, TX, TY>::NT, NDIM == 3 ? 1 : 2)   // 2D: two single-plane blocks per SM overlap their barriers
 #endif
 ark_k_step(const ArkParams P, const double* __restrict__ Uin, double* __restrict__ Uout,
            double dt_value, const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk ARK_TMAP_PARAM) {
