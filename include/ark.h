@@ -89,6 +89,12 @@ int ark_step(ark_solver*, double dt);
  * (ordered with the caller's stream through events): the small 2D configurations are launch-latency-bound. */
 int ark_run(ark_solver*, int nsteps, double cfl, double* dts_out);
 
+/* Diagnostics of the current state as the paper reports them (PAPER.md:398-407 maximum velocity, :435 mean absolute
+ * velocity, :14 conserved mass and total energy).  out (HOST, 6 doubles) = { max |u|, mean |u|, kinetic energy
+ * sum 1/2 rho |u|^2 dV, max Mach number |u|/c, mass sum rho dV, total energy sum (E + rho Phi) dV } with Phi = -g.x
+ * at the cell centres and dV = dx^ndim.  Two-pass reduction without atomics (bit-reproducible); synchronises. */
+int ark_diagnostics(ark_solver*, double* out);
+
 /* Ghost fill only, then copy the PADDED current state ((nx+4)*(ny+4)*(nz+4 or 1) per field, x fastest)
  * to device arrays: test hook for the boundary kernel.  Asynchronous. */
 int ark_debug_get_padded(ark_solver*, double* rho, double* rhou, double* rhov, double* rhow, double* E);

@@ -483,6 +483,37 @@ int oracle_fill_ghosts(int nx, int ny, int nz, double h, double gamma, const dou
     return 0;
 }
 
+// Diagnostics the paper reports (PAPER.md:398-407 maximum velocity, :435 mean absolute velocity, :14 mass and total
+// energy).  out = { max |u|, mean |u|, sum 1/2 rho |u|^2 dV, max |u|/c, sum rho dV, sum (E + rho Phi) dV },
+// Phi = -g.x at the cell centres, dV = h^ndim.  Plain loops, long double accumulators.
+void oracle_diagnostics(int nx, int ny, int nz, double h, double gamma, const double* g,
+                        const double* rho, const double* rhou, const double* rhov, const double* rhow, const double* E,
+                        double* out) {
+    const int ndim = nz == 1 ? 2 : 3;
+    long double s_speed = 0, s_ke = 0, s_m = 0, s_e = 0;
+    double max_speed = 0.0, max_mach = 0.0;
+    size_t j = 0;
+    for (int k = 0; k < nz; ++k) for (int jy = 0; jy < ny; ++jy) for (int i = 0; i < nx; ++i, ++j) {
+        const double mz = (ndim == 3 && rhow) ? rhow[j] : 0.0;
+        const CellPrim w = cons_to_prim(gamma, rho[j], rhou[j], rhov[j], mz, E[j]);
+        const double speed = std::sqrt(w.u[0] * w.u[0] + w.u[1] * w.u[1] + w.u[2] * w.u[2]);
+        const double phi = -(g[0] * (i + 0.5) * h + g[1] * (jy + 0.5) * h + (ndim == 3 ? g[2] * (k + 0.5) * h : 0.0));
+        max_speed = std::max(max_speed, speed);
+        max_mach = std::max(max_mach, speed / w.c);
+        s_speed += speed;
+        s_ke += 0.5 * w.rho * speed * speed;
+        s_m += w.rho;
+        s_e += E[j] + w.rho * phi;
+    }
+    const double vol = ndim == 3 ? h * h * h : h * h;
+    out[0] = max_speed;
+    out[1] = (double)(s_speed / (long double)((size_t)nx * ny * nz));
+    out[2] = (double)(s_ke * vol);
+    out[3] = max_mach;
+    out[4] = (double)(s_m * vol);
+    out[5] = (double)(s_e * vol);
+}
+
 // One acoustic face from primitive L/R data (pin P8).  out = {cL, cR, a, S, u*, theta, Pi*}.
 void oracle_face(double gamma, double rhoL, double unL, double pL, double rhoR, double unR, double pR,
                  double gh, int theta_flag, double* out) {

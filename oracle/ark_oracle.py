@@ -32,6 +32,8 @@ def lib():
         _lib.oracle_face.argtypes = [C.c_double] * 8 + [C.c_int, _dp]
         _lib.oracle_face.restype = None
         _lib.oracle_K.restype = C.c_double
+        _lib.oracle_diagnostics.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _dp] + [_dp] * 5 + [_dp]
+        _lib.oracle_diagnostics.restype = None
     return _lib
 
 
@@ -103,6 +105,16 @@ def face(gamma, rhoL, unL, pL, rhoR, unR, pR, gh=0.0, theta_flag=1):
     out = np.zeros(7)
     lib().oracle_face(gamma, rhoL, unL, pL, rhoR, unR, pR, gh, int(theta_flag), _ptr(out))
     return dict(zip(["cL", "cR", "a", "S", "ustar", "theta", "pistar"], out.tolist()))
+
+
+def diagnostics(p, U):
+    """-> dict(max_speed, mean_speed, kinetic_energy, max_mach, mass, total_energy), see oracle_diagnostics."""
+    S = _state(p, U)
+    g = np.ascontiguousarray(p["g"], dtype=np.float64)
+    out = np.zeros(6)
+    lib().oracle_diagnostics(int(p["nx"]), int(p["ny"]), int(p["nz"]), float(p["dx"]), float(p["gamma"]), _ptr(g),
+                             *[_ptr(a) for a in S], _ptr(out))
+    return dict(zip(("max_speed", "mean_speed", "kinetic_energy", "max_mach", "mass", "total_energy"), out.tolist()))
 
 
 def K():

@@ -16,7 +16,7 @@ ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
 BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
-           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_debug_get_padded",
+           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
 
 
@@ -55,6 +55,8 @@ def load():
     lib.ark_compute_dt.restype = ip
     lib.ark_step.argtypes = [vp, C.c_double]
     lib.ark_step.restype = ip
+    lib.ark_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
+    lib.ark_diagnostics.restype = ip
     lib.ark_run.argtypes = [vp, ip, C.c_double, C.POINTER(C.c_double)]
     lib.ark_run.restype = ip
     lib.ark_step_kernel_timing.argtypes = [vp, ip]
@@ -180,6 +182,12 @@ class Solver:
             return list(buf)[:nsteps]
         _check(self._lib.ark_run(self._h, int(nsteps), float(cfl), None))
         return None
+
+    def diagnostics(self):
+        """-> dict(max_speed, mean_speed, kinetic_energy, max_mach, mass, total_energy) of the current state."""
+        buf = (C.c_double * 6)()
+        _check(self._lib.ark_diagnostics(self._h, buf))
+        return dict(zip(("max_speed", "mean_speed", "kinetic_energy", "max_mach", "mass", "total_energy"), list(buf)))
 
     def step_kernel_timing(self, enable=True):
         _check(self._lib.ark_step_kernel_timing(self._h, int(bool(enable))))

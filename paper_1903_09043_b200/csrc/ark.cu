@@ -32,6 +32,7 @@ constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
 constexpr int CFL_BLOCK = 256;
 #define ARK_MAX_TIMED 4096
 constexpr int MAX_SCRATCH = 1 << 16;          // per-block rate slots
+constexpr int DIAG_BLOCKS = 1184;             // ark_diagnostics: partials live in the last DIAG_BLOCKS * 6 rate slots
 
 size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -295,7 +296,7 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
         s->zchunk = 1;
         s->step_grid = dim3((nx + TX2 - 1) / TX2, (ny + TY2 - 1) / TY2, 1);
     }
-    if ((long long)s->step_grid.x * s->step_grid.y * s->step_grid.z > MAX_SCRATCH) {
+    if ((long long)s->step_grid.x * s->step_grid.y * s->step_grid.z > MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG) {
         delete s;
         return fail(ARK_EINVAL, "ark_create: grid too large for the rate scratch%s");
     }
@@ -507,6 +508,30 @@ int ark_run(ark_solver* s, int nsteps, double cfl, double* dts_out) {
             if (!(dts_out[i] > 0.0) || std::isinf(dts_out[i]))
                 return fail(ARK_ENONFINITE, "ark_run: non-finite CFL rate at step %s%lld", "", (long long)i);
     }
+    return ARK_OK;
+}
+
+int ark_diagnostics(ark_solver* s, double* out) {
+    if (!s || !out) return fail(ARK_EINVAL, "ark_diagnostics: NULL argument%s");
+    const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
+    const int nb = grid_for(n, 256, DIAG_BLOCKS);
+    double* part = s->scratch + (MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG);     // tail of the rate scratch (see ark_create)
+    double* res = s->result + 8;
+    ark_k_diag_pass1<<<nb, 256, 0, s->stream>>>(s->P, s->U[s->cur], part);
+    ark_k_diag_pass2<<<1, 256, 0, s->stream>>>(part, nb, res);
+    s->launches += 2;
+    ARK_CUDA(cudaGetLastError());
+    double h[ARK_NDIAG];
+    ARK_CUDA(cudaMemcpyAsync(h, res, sizeof h, cudaMemcpyDeviceToHost, s->stream));
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    double vol = 1.0;
+    for (int d = 0; d < s->P.ndim; ++d) vol *= s->P.h;
+    out[0] = h[0];                 // max |u|
+    out[1] = h[1] / (double)n;     // mean |u|
+    out[2] = h[2] * vol;           // kinetic energy
+    out[3] = h[3];                 // max Mach number
+    out[4] = h[4] * vol;           // mass
+    out[5] = h[5] * vol;           // total energy incl. potential
     return ARK_OK;
 }
 

@@ -397,6 +397,65 @@ ARK_GLOBAL void ark_k_cfl_pass1(ArkParams P, const double* __restrict__ U, doubl
     if (threadIdx.x == 0) scratch[blockIdx.x] = m;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Diagnostics the paper reports (PAPER.md:398-407 maximum velocity, :435 mean absolute velocity, :14 conserved mass
+// and total energy): max |u|, sum |u|, sum 1/2 rho |u|^2, max Mach, sum rho, sum (E + rho Phi), Phi = -g.x at the
+// cell centres.  Two passes without atomics: fixed grid-stride order per thread, fixed shuffle tree per block, one
+// block over the per-block partials -- the result is bit-reproducible for a given grid.
+// ------------------------------------------------------------------------------------------------
+#define ARK_NDIAG 6
+ARK_DEV void ark_diag_combine(double* a, const double* b) {
+    a[0] = ark_nanmax(a[0], b[0]); a[1] += b[1]; a[2] += b[2]; a[3] = ark_nanmax(a[3], b[3]); a[4] += b[4]; a[5] += b[5];
+}
+ARK_DEV void ark_diag_block(double* v, double* red /* 32 * ARK_NDIAG doubles of shared memory */) {
+#ifndef ARK_HOST_EMU
+    double o[ARK_NDIAG];
+    for (int d = 16; d > 0; d >>= 1) {
+        for (int f = 0; f < ARK_NDIAG; ++f) o[f] = __shfl_down_sync(0xffffffffu, v[f], d);
+        ark_diag_combine(v, o);
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __syncthreads();
+    if (lane == 0) for (int f = 0; f < ARK_NDIAG; ++f) red[wid * ARK_NDIAG + f] = v[f];
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int w2 = 1; w2 < nw; ++w2) ark_diag_combine(v, red + w2 * ARK_NDIAG);
+#else
+    (void)v; (void)red;
+#endif
+}
+ARK_GLOBAL void ark_k_diag_pass1(ArkParams P, const double* __restrict__ U, double* __restrict__ part) {
+    ARK_SHARED double red[32 * ARK_NDIAG];
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    const long long fE = (long long)(P.nf - 1) * P.fstride;
+    double v[ARK_NDIAG] = {0, 0, 0, 0, 0, 0};
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(s % P.nx);
+        const long long r = s / P.nx;
+        const int j = (int)(r % P.ny), k = (int)(r / P.ny);
+        const long long c = ark_idx(P, i, j, k);
+        const double rho = U[c], mx = U[P.fstride + c], my = U[2 * P.fstride + c], mz = P.ndim == 3 ? U[3 * P.fstride + c] : 0.0;
+        const double E = U[fE + c];
+        const double rinv = 1.0 / rho;
+        const double m2 = mx * mx + my * my + mz * mz;
+        const double ke = 0.5 * m2 * rinv;
+        const double speed = sqrt(m2) * rinv;
+        const double cs = sqrt(P.gamma * P.gm1 * (E - ke) * rinv);
+        const double phi = -((i + 0.5) * P.g[0] + (j + 0.5) * P.g[1] + (P.ndim == 3 ? (k + 0.5) * P.g[2] : 0.0)) * P.h;
+        const double w[ARK_NDIAG] = {speed, speed, ke, speed / cs, rho, E + rho * phi};
+        ark_diag_combine(v, w);
+    }
+    ark_diag_block(v, red);
+    if (threadIdx.x == 0) for (int f = 0; f < ARK_NDIAG; ++f) part[(long long)blockIdx.x * ARK_NDIAG + f] = v[f];
+}
+ARK_GLOBAL void ark_k_diag_pass2(const double* __restrict__ part, int nblocks, double* __restrict__ out) {
+    ARK_SHARED double red[32 * ARK_NDIAG];
+    double v[ARK_NDIAG] = {0, 0, 0, 0, 0, 0};
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) ark_diag_combine(v, part + (long long)b * ARK_NDIAG);
+    ark_diag_block(v, red);
+    if (threadIdx.x == 0) for (int f = 0; f < ARK_NDIAG; ++f) out[f] = v[f];
+}
+
 // pass 2: single block over the per-block values; result[0] = max rate,
 // result[1] = dt = cfl / max rate (used by the device-side time loop of ark_run).  With dt_log the step size is also
 // appended at dt_log[*log_count] (a device-side counter, so that the launch can be replayed from a CUDA graph).

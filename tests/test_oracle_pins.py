@@ -642,3 +642,33 @@ def test_flux_wall_feeding_the_conductive_flux_keeps_the_polytrope_at_rest():
     # a flux wall reflects the velocity (free slip): the rest state must survive it as it does the no-slip wall
     assert max(np.abs(S[1] / S[0]).max(), np.abs(S[2] / S[0]).max()) < 1e-12
     assert np.max(np.abs(S[4] - U[4].reshape(-1)) / U[4].reshape(-1)) < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------- diagnostics
+def test_diagnostics_closed_forms():
+    """PAPER.md:398-407 (maximum velocity), :435 (mean absolute velocity), :14 (mass, total energy).  Uniform state under
+    gravity: every entry has a closed form (sum of cell-centre heights = n L / 2); a single fast cell moves the two
+    maxima and nothing else by more than its own share."""
+    nx, ny, nz, h, gamma = 6, 5, 4, 0.25, 1.4
+    rho, u, v, w, p = 1.25, 0.3, -0.4, 1.2, 0.75
+    g = (0.0, 0.5, -2.0)
+    prm = I.make_params(nx, ny, nz, h, gamma, g=g)
+    E = p / (gamma - 1) + 0.5 * rho * (u * u + v * v + w * w)
+    U = [np.full((nz, ny, nx), x) for x in (rho, rho * u, rho * v, rho * w, E)]
+    d = O.diagnostics(prm, U)
+    speed = math.sqrt(u * u + v * v + w * w)          # = 1.3
+    V = nx * ny * nz * h ** 3
+    assert abs(d["max_speed"] - speed) < 1e-15 and abs(d["mean_speed"] - speed) < 1e-15
+    assert abs(d["kinetic_energy"] - 0.5 * rho * speed ** 2 * V) < 1e-13
+    assert abs(d["max_mach"] - speed / math.sqrt(gamma * p / rho)) < 1e-15
+    assert abs(d["mass"] - rho * V) < 1e-13
+    # Phi = -g.x: mean height of the cell centres along an axis of n cells is n h / 2
+    phi_mean = -(g[1] * ny * h / 2 + g[2] * nz * h / 2)
+    assert abs(d["total_energy"] - (E + rho * phi_mean) * V) < 1e-12
+    s2 = math.sqrt(u * u + v * v + 25.0)
+    U[3][2, 1, 3] = rho * 5.0                          # one fast cell at the same pressure
+    U[4][2, 1, 3] = p / (gamma - 1) + 0.5 * rho * s2 * s2
+    d2 = O.diagnostics(prm, U)
+    assert abs(d2["max_speed"] - s2) < 1e-14
+    assert abs(d2["mean_speed"] - (speed * (nx * ny * nz - 1) + s2) / (nx * ny * nz)) < 1e-14
+    assert abs(d2["max_mach"] - s2 / math.sqrt(gamma * p / rho)) < 1e-13 and abs(d2["mass"] - d["mass"]) < 1e-13

@@ -359,3 +359,22 @@ def test_parity_extreme_aspect_ratios(B, shape):
     ref, dts = O.run(prm, U, 4, cfl=0.4)
     got = gpu_run(B, prm, U, dts)
     assert max(rel_err(ref, got)) < 1e-12, (shape, rel_err(ref, got))
+
+
+def test_diagnostics_match_oracle(B):
+    """max |u|, mean |u|, kinetic energy, max Mach, mass, total energy after a few steps:
+    maxima to 1e-13, sums to 1e-12 (tree vs sequential order), and the reduction is bit-reproducible."""
+    for name in ("3d_walls_viscous", "2d_walls_gravity_viscous", "3d_periodic"):
+        prm, U = RANDOM[name]()
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        s.run(3, 0.4)
+        got = s.diagnostics()
+        again = s.diagnostics()
+        out = to_np(s.get_state())
+        s.close()
+        assert got == again
+        ref = O.diagnostics(prm, out)                    # the oracle's formulas on the SAME state
+        for k, tol in (("max_speed", 1e-13), ("max_mach", 1e-13), ("mean_speed", 1e-12), ("kinetic_energy", 1e-12),
+                       ("mass", 1e-12), ("total_energy", 1e-12)):
+            assert abs(got[k] - ref[k]) <= tol * abs(ref[k]), (name, k, got[k], ref[k])
