@@ -408,3 +408,35 @@ def test_baseline_configs_full_step_counts(B):
         d = s.diagnostics()
         s.close()
         assert d["max_speed"] < 1e-12, (prm["nx"], d)
+
+
+def test_3d_baseline_configs_full_step_counts(B):
+    """config 4 (256^3, 200 steps) and config 5 (512^3, 50 steps) at full size through the device-side loop: mass conserved
+    to round-off; config 5's total energy grows by exactly the imposed bottom flux (reading A22: F x wall area x time, the
+    top wall is insulating and no mass crosses a wall), config 4 stays subsonic and finite."""
+    prm, U = I.config4_rb3d(256, device="cuda")
+    s = B.Solver(prm)
+    s.set_state([a.reshape(-1) for a in U])
+    d0 = s.diagnostics()
+    s.run(200, 0.4)
+    d1 = s.diagnostics()
+    s.close()
+    assert abs(d1["mass"] - d0["mass"]) < 1e-12 * d0["mass"]
+    assert 0.0 < d1["max_mach"] < 0.1 and np.isfinite(d1["total_energy"])
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40e9:
+        pytest.skip("not enough device memory for 512^3")
+    del U
+    prm, U = I.config5_convection3d(512, device="cuda")
+    s = B.Solver(prm)
+    s.set_state([a.reshape(-1) for a in U])
+    del U
+    d0 = s.diagnostics()
+    dts = s.run(50, 0.4, want_dts=True)
+    d1 = s.diagnostics()
+    s.close()
+    F = prm["bc_value"][2][0]
+    assert prm["bc_type"][2] == (I.BC_FLUX, REF) and F > 0
+    assert abs(d1["mass"] - d0["mass"]) < 1e-12 * d0["mass"]
+    gain = d1["total_energy"] - d0["total_energy"]
+    assert abs(gain - F * 1.0 * sum(dts)) < 2e-12 * abs(d0["total_energy"]), (gain, F * sum(dts), d0["total_energy"])
