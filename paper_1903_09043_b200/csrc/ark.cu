@@ -9,7 +9,7 @@
 #include <cstring>
 #include <new>
 
-#include "ark_step.cuh"
+#include "ark_step3d.cuh"
 
 namespace {
 
@@ -26,7 +26,8 @@ int fail(int code, const char* fmt, const char* a = "", long long b = 0) {
     } while (0)
 
 // tile of the fused step kernel
-constexpr int TX3 = ARK_TX3, TY3 = ARK_TY3;   // 3D
+constexpr int TX3 = ARK_TX3, NW3 = ARK_NW3;   // 3D: outputs per row, row pairs per block
+constexpr int TY3 = 2 * NW3 - 4;
 constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
 
 constexpr int CFL_BLOCK = 256;
@@ -138,12 +139,7 @@ int grid_for(long long n, int block, int cap = 148 * 8) {
 template <int NDIM, bool VISC, int TX, int TY>
 int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
     using C = ArkStepCfg<NDIM, VISC, TX, TY>;
-    static bool attr_set = false;
     auto kern = ark_k_step<NDIM, VISC, TX, TY>;
-    if (!attr_set) {
-        ARK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-        attr_set = true;
-    }
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
     if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
     kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
@@ -177,12 +173,45 @@ int launch_bc(ark_solver* s, double* U) {
     return ARK_OK;
 }
 
+template <bool VISC, bool GXY>
+int launch_step3(ark_solver* s, double dt, const double* dt_dev) {
+    using C = ArkCfg3<VISC, TX3, NW3>;
+    auto kern = ark_k_step3<VISC, GXY, TX3, NW3>;
+    const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
+    if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
+    kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
+                                                            s->scratch, s->zchunk, s->tmap[s->cur]);
+    if (timed) { ARK_CUDA(cudaEventRecord(s->ev1[s->n_timed], s->stream)); s->n_timed++; }
+    ARK_CUDA(cudaGetLastError());
+    s->launches++;
+    return ARK_OK;
+}
+
+// opt-in to the large dynamic shared memory of the step kernels on the CURRENT device (the attribute is per device)
+int set_step_attributes(int ndim) {
+    if (ndim == 3) {
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<true, true, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<true, TX3, NW3>::SMEM_BYTES));
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<true, false, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<true, TX3, NW3>::SMEM_BYTES));
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<false, true, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<false, TX3, NW3>::SMEM_BYTES));
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<false, false, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<false, TX3, NW3>::SMEM_BYTES));
+    } else {
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step<2, true, TX2, TY2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkStepCfg<2, true, TX2, TY2>::SMEM_BYTES));
+        ARK_CUDA(cudaFuncSetAttribute(ark_k_step<2, false, TX2, TY2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkStepCfg<2, false, TX2, TY2>::SMEM_BYTES));
+    }
+    return ARK_OK;
+}
+
 int do_step(ark_solver* s, double dt, const double* dt_dev) {
     int rc = launch_bc(s, s->U[s->cur]);
     if (rc != ARK_OK) return rc;
     const bool visc = s->P.mu > 0.0 || s->P.kappa > 0.0;
-    if (s->P.ndim == 3) rc = visc ? launch_step_t<3, true, TX3, TY3>(s, dt, dt_dev) : launch_step_t<3, false, TX3, TY3>(s, dt, dt_dev);
-    else                rc = visc ? launch_step_t<2, true, TX2, TY2>(s, dt, dt_dev) : launch_step_t<2, false, TX2, TY2>(s, dt, dt_dev);
+    if (s->P.ndim == 3) {
+        const bool gxy = s->P.D.g_on[0] || s->P.D.g_on[1];
+        if (visc) rc = gxy ? launch_step3<true, true>(s, dt, dt_dev) : launch_step3<true, false>(s, dt, dt_dev);
+        else      rc = gxy ? launch_step3<false, true>(s, dt, dt_dev) : launch_step3<false, false>(s, dt, dt_dev);
+    } else {
+        rc = visc ? launch_step_t<2, true, TX2, TY2>(s, dt, dt_dev) : launch_step_t<2, false, TX2, TY2>(s, dt, dt_dev);
+    }
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
     s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
@@ -214,8 +243,8 @@ const char* ark_last_error(void) { return g_err; }
 
 const char* ark_version_string(void) {
     static char buf[256];
-    snprintf(buf, sizeof buf, "ark-b200 0.1 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d tile2d=%dx%d)", ARK_K_IMPEDANCE, ARK_NG,
-             TX3, TY3, TX2, TY2);
+    snprintf(buf, sizeof buf, "ark-b200 0.1 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d (%d row pairs) tile2d=%dx%d)", ARK_K_IMPEDANCE, ARK_NG,
+             TX3, TY3, NW3, TX2, TY2);
     return buf;
 }
 
@@ -306,6 +335,7 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
             if (rc != ARK_OK) { delete s; return rc; }
         }
     }
+    { const int rc = set_step_attributes(ndim); if (rc != ARK_OK) { delete s; return rc; } }
     cudaError_t e = cudaMallocHost((void**)&s->h_pinned, 2 * sizeof(double));
     if (e != cudaSuccess) { delete s; return fail(ARK_ECUDA, "CUDA error: %s", cudaGetErrorString(e)); }
     // ghost cells and padding start finite (they are read by clamped / halo threads before the first fill)

@@ -14,12 +14,14 @@
 #include <cuda.h>           // CUtensorMap (type only; the encoder is fetched through the runtime, see ark.cu)
 #include <cuda_runtime.h>
 #define ARK_DEV __device__ __forceinline__
+#define ARK_HD __host__ __device__
 #define ARK_GLOBAL __global__
 #define ARK_SHARED __shared__
 #define ARK_DYN_SMEM(name) extern __shared__ double name[]
 #else
-// host emulation shim (debugging aid outside the product build): supplies threadIdx & co, __syncthreads, rsqrt
-#include "ark_emu.h"
+// host emulation (tests only): the including translation unit supplies threadIdx & co, __syncthreads, rsqrt and the
+// ARK_* macros BEFORE this header (tests/emu/ark_emu.h); nothing of it is part of the product build
+#define ARK_HD
 #endif
 
 #define ARK_K_IMPEDANCE 1.1  // a = K max(rho_L c_L, rho_R c_R), reading A2
@@ -140,6 +142,64 @@ ARK_DEV void ark_mbar_wait(unsigned long long* bar, unsigned parity) {
         "bra ARK_WAIT_%=;\n"
         "ARK_DONE_%=:\n"
         "}\n" ::"r"(ark_smem_u32(bar)), "r"(parity) : "memory");
+}
+#endif
+
+// ------------------------------------------------------------------------------------------------
+// Tensor memory (TMEM, 256 KB per SM) as a per-thread scratch space.  The step kernel has no tensor-core work, so
+// the whole TMEM of the SM is free: a warp may address lanes 32*(warp%4) .. +31, i.e. thread `lane` of a warp owns
+// one TMEM lane, and the 512 32-bit columns of that lane are split among the warps that share the lane quarter.
+// tcgen05.st / tcgen05.ld (shape 32x32b: one column = one 32-bit word per thread) move registers <-> TMEM on a
+// datapath of their own (measured on B200: > 460 B/clk/SM with 8 warps, ~30 cycles load-to-use), which relieves both
+// the register file (the z pipeline of a column is parked there between its uses) and the shared-memory pipe.
+// A double occupies two adjacent columns.  ark_tm_ld must be followed by ark_tm_wait_ld() before the values are
+// used; ark_tm_wait_st() orders earlier stores before later loads of the same columns.
+// ------------------------------------------------------------------------------------------------
+#ifndef ARK_HOST_EMU
+#define ARK_LO(x) "r"(__double2loint(x))
+#define ARK_HI(x) "r"(__double2hiint(x))
+ARK_DEV unsigned ark_tm_alloc_all(unsigned* slot_in_smem) {           // one full warp; 512 columns = the whole TMEM
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(ark_smem_u32(slot_in_smem)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    return 0;
+}
+ARK_DEV void ark_tm_free_all(unsigned base) {                         // the same warp that allocated
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
+ARK_DEV void ark_tm_fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+ARK_DEV void ark_tm_fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+ARK_DEV void ark_tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+ARK_DEV void ark_tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+ARK_DEV void ark_tm_st1(unsigned a, double v0) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(a), ARK_LO(v0), ARK_HI(v0) : "memory");
+}
+ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1),
+                 ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3) : "memory");
+}
+ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(a),
+                 ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3), ARK_LO(v4), ARK_HI(v4),
+                 ARK_LO(v5), ARK_HI(v5), ARK_LO(v6), ARK_HI(v6), ARK_LO(v7), ARK_HI(v7) : "memory");
+}
+ARK_DEV void ark_tm_ld1(unsigned a, double& v0) {
+    int l0, h0;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(l0), "=r"(h0) : "r"(a) : "memory");
+    v0 = __hiloint2double(h0, l0);
+}
+ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) {
+    int l0, h0, l1, h1, l2, h2, l3, h3;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3) : "r"(a) : "memory");
+    v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
+}
+ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
+    int l0, h0, l1, h1, l2, h2, l3, h3, l4, h4, l5, h5, l6, h6, l7, h7;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3), "=r"(l4), "=r"(h4), "=r"(l5), "=r"(h5),
+                   "=r"(l6), "=r"(h6), "=r"(l7), "=r"(h7) : "r"(a) : "memory");
+    v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
+    v4 = __hiloint2double(h4, l4); v5 = __hiloint2double(h5, l5); v6 = __hiloint2double(h6, l6); v7 = __hiloint2double(h7, l7);
 }
 #endif
 

@@ -16,7 +16,8 @@ _lib = None
 def build():
     srcs = [os.path.join(HERE, "emu_driver.cpp"), os.path.join(HERE, "ark_emu.h"),
             os.path.join(ROOT, "paper_1903_09043_b200", "csrc", "ark_device.cuh"),
-            os.path.join(ROOT, "paper_1903_09043_b200", "csrc", "ark_step.cuh")]
+            os.path.join(ROOT, "paper_1903_09043_b200", "csrc", "ark_step.cuh"),
+            os.path.join(ROOT, "paper_1903_09043_b200", "csrc", "ark_step3d.cuh")]
     if os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in srcs):
         return LIB
     subprocess.run(["g++", "-std=c++20", "-O1", "-ffp-contract=off", "-fPIC", "-shared", "-pthread",

@@ -3,13 +3,16 @@
 // (pack, ghost fill x/y/z, fused step, unpack; standalone CFL passes) with a small tile so that a tiny grid
 // still spans several tiles, a ragged tail and several z chunks.
 #define ARK_HOST_EMU 1
+#define ARK_REG_RING 96
+#define ARK_REG_TILE 208
 #include "ark_emu.h"
-#include "../../paper_1903_09043_b200/csrc/ark_step.cuh"
+#include "../../paper_1903_09043_b200/csrc/ark_step3d.cuh"
 
 #include <cstring>
 
 namespace {
 constexpr int ETX = 8, ETY = 4;   // emulation tile
+constexpr int ENW = 4;            // 3D: row pairs per block (region 12 x 8, tile 8 x 4) on ENW + 2 "warps" of 12 threads
 
 ArkParams make_params(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa,
                       int theta, const int* bt, const double* bv) {
@@ -35,8 +38,16 @@ void bc(const ArkParams& P, double* U, long long n) {
 
 template <int NDIM, bool VISC>
 void step(const ArkParams& P, const double* Uin, double* Uout, double dt, double* scratch, int zchunk, emu_dim3 grid) {
-    using C = ArkStepCfg<NDIM, VISC, ETX, ETY>;
-    ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch, zchunk); });
+    if constexpr (NDIM == 3) {
+        using C = ArkCfg3<VISC, ETX, ENW>;
+        static_assert(C::TY == ETY, "emulation tile");
+        const bool gxy = P.D.g_on[0] || P.D.g_on[1];
+        if (gxy) ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, true, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
+        else     ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, false, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
+    } else {
+        using C = ArkStepCfg<NDIM, VISC, ETX, ETY>;
+        ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch, zchunk); });
+    }
 }
 }  // namespace
 
