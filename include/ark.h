@@ -18,6 +18,8 @@
  *     ark_workspace_bytes() bytes, 256-byte aligned; it must outlive the handle.
  *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call
  *     enqueues on that stream; only the calls documented as synchronising wait for it.
+ *   - A handle belongs to the CUDA device that was current in ark_create (its workspace, stream and kernel
+ *     attributes live there): calling an entry point while another device is current returns ARK_EINVAL.
  *   - Every entry point returns an ARK_* code and never throws; ark_last_error() gives a text for
  *     the last failure on the calling thread.
  *   - Gravity is the constant vector g (Phi = -g.x, never stored: A12).  The acoustic impedance
@@ -48,7 +50,9 @@ typedef struct {
                            is reflected as at a reflecting wall; needs kappa > 0.  Ignored otherwise. */
 } ark_bc;
 
-/* Bytes of device workspace ark_create needs for an nx*ny*nz grid (0 if the sizes are invalid). */
+/* Bytes of device workspace ark_create needs for an nx*ny*nz grid; 0 if the sizes are invalid (nx,ny >= 4, nz == 1 or
+ * >= 4, each <= 16384) or if the grid needs more fused-step blocks than the per-block rate scratch holds (58 432:
+ * e.g. 2D 4096^2 is too large, 2D 2048^2 and 3D 1024^3 fit); ark_create rejects the same grids with ARK_EINVAL. */
 size_t ark_workspace_bytes(int nx, int ny, int nz);
 
 /* Create a solver.  nx,ny >= 4; nz >= 4 or nz == 1 (2D).  dx > 0 (uniform); gamma > 1
@@ -84,7 +88,9 @@ int ark_step(ark_solver*, double dt);
 
 /* Convenience: nsteps x { dt = cfl / max rate ; step(dt) } with the time step kept on the device
  * (no host round trip per step).  If dts_out (HOST, nsteps doubles) is not NULL the step sizes are
- * copied there; the call then synchronises.  Returns ARK_ENONFINITE if a rate was not finite.
+ * copied there.  The call synchronises the stream ONCE, after the last step, to read a sticky device-side flag:
+ * it returns ARK_ENONFINITE if any maximum rate of the run was not finite and positive (the remaining steps of such a
+ * run have consumed a NaN step size; the state is then meaningless), with or without dts_out.
  * After the first step, pairs of steps are replayed from a CUDA graph captured on a stream of the library's own
  * (ordered with the caller's stream through events): the small 2D configurations are launch-latency-bound. */
 int ark_run(ark_solver*, int nsteps, double cfl, double* dts_out);

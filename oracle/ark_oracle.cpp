@@ -183,7 +183,15 @@ void fill_ghosts(const Cfg& cfg, const Grid& G, State& U) {
                     // delta = Phi_prev - Phi_ghost, Phi = -g.x
                     const double delta = (side == 0 ? -1.0 : 1.0) * cfg.g[d] * cfg.h;
                     // eq. (14) with p_g = rho_g T_g:  rho_g = (p_prev + 1/2 rho_prev delta)/(T_g - 1/2 delta)
-                    const double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
+                    double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
+                    // reading A9 requires T_g > |g_d| h / 2; without it relation (14) has no positive solution and the
+                    // wall closure is undefined: the ghost cell is flagged (NaN), which compute_dt reports as non-finite
+                    // (only ghost cells that face interior cells: edge / corner ghosts mirror ghost cells of another
+                    // wall, their doubly mirrored temperature carries no physical meaning and only their velocity is
+                    // ever used, by the diagonal points of the viscous stencil)
+                    bool faces_interior = true;
+                    for (int e = 0; e < cfg.ndim; ++e) if (e != d && (c[e] < 0 || c[e] >= G.n[e])) faces_interior = false;
+                    if (faces_interior && !(rg > 0.0)) rg = std::nan("");
                     const double pg = rg * Tg;
                     U.q[0][jg] = rg;
                     U.q[1][jg] = rg * ug[0];

@@ -83,6 +83,7 @@ struct ark_solver {
     double* stage;
     cudaStream_t stream;
     int rate_slots;         // >0: scratch[0..rate_slots) holds the per-block rates of the CURRENT state
+    bool xghost_valid;      // 3D, periodic x: the step kernel already wrote the x ghost columns of the current state
     dim3 step_grid;
     int zchunk;
     long long launches;
@@ -96,12 +97,14 @@ struct ark_solver {
     double g_cfl;
     long long g_launches;   // kernel launches inside one replay
     double* h_pinned;       // 2 doubles, pinned, for the 16-byte D2H of compute_dt
-    // optional event bracketing of the step kernel (measurement hook)
+    int device;             // the CUDA device the handle was created on (entry points check it is current)
+    // optional event bracketing of the step kernel (measurement hook): allocated on first use, outside the handle
     bool timing;
     int n_timed;
-    cudaEvent_t ev0[ARK_MAX_TIMED], ev1[ARK_MAX_TIMED];
-    bool ev_created;
+    struct ArkTimer* timer;
 };
+
+struct ArkTimer { cudaEvent_t ev0[ARK_MAX_TIMED], ev1[ARK_MAX_TIMED]; };
 
 namespace {
 
@@ -130,6 +133,15 @@ int make_tensor_map(CUtensorMap* out, const Layout& L, double* base, int rx, int
     return ARK_OK;
 }
 
+// every entry point runs on the device the handle was created on
+int check_device(const ark_solver* s) {
+    int dev = -1;
+    ARK_CUDA(cudaGetDevice(&dev));
+    if (dev != s->device) return fail(ARK_EINVAL, "the solver was created on CUDA device %s%lld, which is not the current device", "", (long long)s->device);
+    return ARK_OK;
+}
+#define ARK_ON_DEVICE(s) do { const int rc_ = check_device(s); if (rc_ != ARK_OK) return rc_; } while (0)
+
 int grid_for(long long n, int block, int cap = 148 * 8) {
     long long b = (n + block - 1) / block;
     if (b < 1) b = 1;
@@ -141,10 +153,10 @@ int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
     using C = ArkStepCfg<NDIM, VISC, TX, TY>;
     auto kern = ark_k_step<NDIM, VISC, TX, TY>;
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
-    if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
+    if (timed) ARK_CUDA(cudaEventRecord(s->timer->ev0[s->n_timed], s->stream));
     kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
                                                             s->scratch, s->zchunk, s->tmap[s->cur]);
-    if (timed) { ARK_CUDA(cudaEventRecord(s->ev1[s->n_timed], s->stream)); s->n_timed++; }
+    if (timed) { ARK_CUDA(cudaEventRecord(s->timer->ev1[s->n_timed], s->stream)); s->n_timed++; }
     ARK_CUDA(cudaGetLastError());
     s->launches++;
     return ARK_OK;
@@ -153,17 +165,23 @@ int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
 int launch_bc(ark_solver* s, double* U) {
     const ArkParams& P = s->P;
     if (P.bc[0][0] == ARK_BCK_PERIODIC) {
-        const long long n = 2LL * P.ny * P.nz * P.nf;
-        ark_k_bc_x_periodic<<<grid_for(n, 256, 148 * 16), 256, 0, s->stream>>>(P, U);
+        // (3D: the fused step kernel writes the periodic x ghost columns of the state it produces; the sweep is only
+        // needed for a state that came from outside)
+        if (!s->xghost_valid) {
+            const long long n = 2LL * P.ny * P.nz * P.nf;
+            ark_k_bc_x_periodic<<<grid_for(n, 256, 148 * 16), 256, 0, s->stream>>>(P, U);
+            s->launches++;
+        }
     } else {
         const long long n = 2LL * P.ny * P.nz;
         ark_k_bc<0><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
+        s->launches++;
     }
     {
         const long long n = 2LL * (P.nx + 2 * ARK_NG) * P.nz;
         ark_k_bc<1><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
+        s->launches++;
     }
-    s->launches += 2;
     if (P.ndim == 3) {
         const long long n = 2LL * (P.nx + 2 * ARK_NG) * (P.ny + 2 * ARK_NG);
         ark_k_bc<2><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
@@ -178,10 +196,10 @@ int launch_step3(ark_solver* s, double dt, const double* dt_dev) {
     using C = ArkCfg3<VISC, TX3, NW3>;
     auto kern = ark_k_step3<VISC, GXY, TX3, NW3>;
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
-    if (timed) ARK_CUDA(cudaEventRecord(s->ev0[s->n_timed], s->stream));
+    if (timed) ARK_CUDA(cudaEventRecord(s->timer->ev0[s->n_timed], s->stream));
     kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
                                                             s->scratch, s->zchunk, s->tmap[s->cur]);
-    if (timed) { ARK_CUDA(cudaEventRecord(s->ev1[s->n_timed], s->stream)); s->n_timed++; }
+    if (timed) { ARK_CUDA(cudaEventRecord(s->timer->ev1[s->n_timed], s->stream)); s->n_timed++; }
     ARK_CUDA(cudaGetLastError());
     s->launches++;
     return ARK_OK;
@@ -214,6 +232,7 @@ int do_step(ark_solver* s, double dt, const double* dt_dev) {
     }
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
+    s->xghost_valid = s->P.ndim == 3 && s->P.bc[0][0] == ARK_BCK_PERIODIC;
     s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
     return ARK_OK;
 }
@@ -248,8 +267,45 @@ const char* ark_version_string(void) {
     return buf;
 }
 
+}  // extern "C"
+
+namespace {
+
+// number of blocks of the fused step kernel (= per-block CFL rate slots it fills)
+long long step_blocks(int nx, int ny, int nz, dim3* grid, int* zchunk) {
+    if (nz > 1) {
+        const int gx = (nx + TX3 - 1) / TX3, gy = (ny + TY3 - 1) / TY3;
+        // z chunks: a block marches zc planes (+ ~2.5 planes of prologue) and the grid runs in ceil(blocks / 148)
+        // rounds of one block per SM; pick the chunk count that minimises rounds * (zc + 2.5), chunks >= 16 planes
+        int zc = nz;
+        double best = 1e300;
+        for (int nch = 1; nch <= (nz / 16 > 1 ? nz / 16 : 1); ++nch) {
+            const int c = (nz + nch - 1) / nch;
+            const long long blocks = (long long)gx * gy * ((nz + c - 1) / c);
+            const double cost = (double)((blocks + 147) / 148) * (c + 2.5);
+            if (cost < best) { best = cost; zc = c; }
+        }
+        const int nchunk = (nz + zc - 1) / zc;
+        if (zchunk) *zchunk = zc;
+        if (grid) *grid = dim3(gx, gy, nchunk);
+        return (long long)gx * gy * nchunk;
+    }
+    if (zchunk) *zchunk = 1;
+    const int gx = (nx + TX2 - 1) / TX2, gy = (ny + TY2 - 1) / TY2;
+    if (grid) *grid = dim3(gx, gy, 1);
+    return (long long)gx * gy;
+}
+
+bool supported_grid(int nx, int ny, int nz) {
+    return valid_sizes(nx, ny, nz) && step_blocks(nx, ny, nz, nullptr, nullptr) <= MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG;
+}
+
+}  // namespace
+
+extern "C" {
+
 size_t ark_workspace_bytes(int nx, int ny, int nz) {
-    if (!valid_sizes(nx, ny, nz)) return 0;
+    if (!supported_grid(nx, ny, nz)) return 0;
     return make_layout(nx, ny, nz).total;
 }
 
@@ -304,30 +360,12 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     s->stream = (cudaStream_t)cuda_stream;
     s->rate_slots = 0;
     s->launches = 0;
+    { cudaError_t e0 = cudaGetDevice(&s->device); if (e0 != cudaSuccess) { delete s; return fail(ARK_ECUDA, "CUDA error: %s", cudaGetErrorString(e0)); } }
 
     // launch geometry of the fused step kernel
-    if (ndim == 3) {
-        const int gx = (nx + TX3 - 1) / TX3, gy = (ny + TY3 - 1) / TY3;
-        // z chunks: a block marches zc planes (+ ~2.5 planes of prologue) and the grid runs in ceil(blocks / 148)
-        // rounds of one block per SM; pick the chunk count that minimises rounds * (zc + 2.5), chunks >= 16 planes
-        int zc = nz;
-        double best = 1e300;
-        for (int nch = 1; nch <= (nz / 16 > 1 ? nz / 16 : 1); ++nch) {
-            const int c = (nz + nch - 1) / nch;
-            const long long blocks = (long long)gx * gy * ((nz + c - 1) / c);
-            const double cost = (double)((blocks + 147) / 148) * (c + 2.5);
-            if (cost < best) { best = cost; zc = c; }
-        }
-        const int nchunk = (nz + zc - 1) / zc;
-        s->zchunk = zc;
-        s->step_grid = dim3(gx, gy, nchunk);
-    } else {
-        s->zchunk = 1;
-        s->step_grid = dim3((nx + TX2 - 1) / TX2, (ny + TY2 - 1) / TY2, 1);
-    }
-    if ((long long)s->step_grid.x * s->step_grid.y * s->step_grid.z > MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG) {
+    if (step_blocks(nx, ny, nz, &s->step_grid, &s->zchunk) > MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG) {
         delete s;
-        return fail(ARK_EINVAL, "ark_create: grid too large for the rate scratch%s");
+        return fail(ARK_EINVAL, "ark_create: grid too large for the per-block rate scratch (ark_workspace_bytes returns 0 for it)%s");
     }
     if (ndim == 3) {
         for (int b = 0; b < 2; ++b) {
@@ -347,12 +385,13 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
 
 int ark_step_kernel_timing(ark_solver* s, int enable) {
     if (!s) return fail(ARK_EINVAL, "ark_step_kernel_timing: NULL handle%s");
-    if (enable && !s->ev_created) {
+    if (enable && !s->timer) {
+        s->timer = new (std::nothrow) ArkTimer;
+        if (!s->timer) return fail(ARK_ENOMEM, "ark_step_kernel_timing: out of host memory%s");
         for (int i = 0; i < ARK_MAX_TIMED; ++i) {
-            ARK_CUDA(cudaEventCreate(&s->ev0[i]));
-            ARK_CUDA(cudaEventCreate(&s->ev1[i]));
+            ARK_CUDA(cudaEventCreate(&s->timer->ev0[i]));
+            ARK_CUDA(cudaEventCreate(&s->timer->ev1[i]));
         }
-        s->ev_created = true;
     }
     s->timing = enable != 0;
     s->n_timed = 0;
@@ -365,7 +404,7 @@ int ark_step_kernel_time(ark_solver* s, double* total_ms, int* launches) {
     double sum = 0.0;
     for (int i = 0; i < s->n_timed; ++i) {
         float ms = 0.f;
-        ARK_CUDA(cudaEventElapsedTime(&ms, s->ev0[i], s->ev1[i]));
+        ARK_CUDA(cudaEventElapsedTime(&ms, s->timer->ev0[i], s->timer->ev1[i]));
         sum += ms;
     }
     *total_ms = sum;
@@ -375,8 +414,10 @@ int ark_step_kernel_time(ark_solver* s, double* total_ms, int* launches) {
 
 void ark_destroy(ark_solver* s) {
     if (!s) return;
-    if (s->ev_created)
-        for (int i = 0; i < ARK_MAX_TIMED; ++i) { cudaEventDestroy(s->ev0[i]); cudaEventDestroy(s->ev1[i]); }
+    if (s->timer) {
+        for (int i = 0; i < ARK_MAX_TIMED; ++i) { cudaEventDestroy(s->timer->ev0[i]); cudaEventDestroy(s->timer->ev1[i]); }
+        delete s->timer;
+    }
     if (s->h_pinned) cudaFreeHost(s->h_pinned);
     if (s->gexec) cudaGraphExecDestroy(s->gexec);
     if (s->gstream) { cudaEventDestroy(s->gev_in); cudaEventDestroy(s->gev_out); cudaStreamDestroy(s->gstream); }
@@ -388,6 +429,7 @@ long long ark_launch_count(const ark_solver* s) { return s ? s->launches : 0; }
 int ark_set_state(ark_solver* s, const double* rho, const double* rhou, const double* rhov, const double* rhow,
                   const double* E) {
     if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_set_state: NULL argument%s");
+    ARK_ON_DEVICE(s);
     const double* src[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
     const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
     for (int f = 0; f < s->P.nf; ++f) {
@@ -396,11 +438,13 @@ int ark_set_state(ark_solver* s, const double* rho, const double* rhou, const do
     }
     ARK_CUDA(cudaGetLastError());
     s->rate_slots = 0;
+    s->xghost_valid = false;
     return ARK_OK;
 }
 
 int ark_get_state(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
     if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_get_state: NULL argument%s");
+    ARK_ON_DEVICE(s);
     double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
     const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
     for (int f = 0; f < s->P.nf; ++f) {
@@ -414,6 +458,7 @@ int ark_get_state(ark_solver* s, double* rho, double* rhou, double* rhov, double
 int ark_set_state_host(ark_solver* s, const double* rho, const double* rhou, const double* rhov, const double* rhow,
                        const double* E) {
     if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_set_state_host: NULL argument%s");
+    ARK_ON_DEVICE(s);
     const double* src[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
     const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
     for (int f = 0; f < s->P.nf; ++f) {
@@ -425,11 +470,13 @@ int ark_set_state_host(ark_solver* s, const double* rho, const double* rhou, con
     ARK_CUDA(cudaGetLastError());
     ARK_CUDA(cudaStreamSynchronize(s->stream));
     s->rate_slots = 0;
+    s->xghost_valid = false;
     return ARK_OK;
 }
 
 int ark_get_state_host(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
     if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_get_state_host: NULL argument%s");
+    ARK_ON_DEVICE(s);
     double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};
     const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
     for (int f = 0; f < s->P.nf; ++f) {
@@ -445,6 +492,7 @@ int ark_get_state_host(ark_solver* s, double* rho, double* rhou, double* rhov, d
 
 int ark_compute_dt(ark_solver* s, double cfl, double* dt_out) {
     if (!s || !dt_out || !(cfl > 0.0)) return fail(ARK_EINVAL, "ark_compute_dt: bad argument%s");
+    ARK_ON_DEVICE(s);
     int rc = reduce_rate(s, cfl, nullptr);
     if (rc != ARK_OK) return rc;
     ARK_CUDA(cudaMemcpyAsync(s->h_pinned, s->result, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
@@ -460,6 +508,7 @@ int ark_compute_dt(ark_solver* s, double cfl, double* dt_out) {
 
 int ark_step(ark_solver* s, double dt) {
     if (!s || !(dt > 0.0) || std::isinf(dt)) return fail(ARK_EINVAL, "ark_step: dt must be finite and positive%s");
+    ARK_ON_DEVICE(s);
     return do_step(s, dt, nullptr);
 }
 
@@ -518,9 +567,11 @@ int run_pairs_graph(ark_solver* s, int npairs, double cfl, double* dt_log) {
 
 int ark_run(ark_solver* s, int nsteps, double cfl, double* dts_out) {
     if (!s || nsteps < 0 || !(cfl > 0.0)) return fail(ARK_EINVAL, "ark_run: bad argument%s");
+    ARK_ON_DEVICE(s);
     if (dts_out && nsteps > DTLOG_MAX) return fail(ARK_EINVAL, "ark_run: at most %s%lld steps when dts_out is given", "", (long long)DTLOG_MAX);
     double* dt_log = dts_out ? s->dtlog : nullptr;
-    if (dts_out) ARK_CUDA(cudaMemsetAsync(s->result + 4, 0, sizeof(int), s->stream));
+    // result[3]: sticky "a rate was not finite and positive" flag of pass 2; result[4]: log counter
+    ARK_CUDA(cudaMemsetAsync(s->result + 3, 0, 2 * sizeof(double), s->stream));
     int done = 0;
     // the first step may need the standalone rate pass; from then on every step has the same launch sequence
     if (nsteps > 0) { const int rc = run_one(s, cfl, dt_log); if (rc != ARK_OK) return rc; done = 1; }
@@ -531,18 +582,19 @@ int ark_run(ark_solver* s, int nsteps, double cfl, double* dts_out) {
         done += 2 * npairs;
     }
     for (; done < nsteps; ++done) { const int rc = run_one(s, cfl, dt_log); if (rc != ARK_OK) return rc; }
-    if (dts_out && nsteps > 0) {
-        ARK_CUDA(cudaMemcpyAsync(dts_out, s->dtlog, (size_t)nsteps * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    if (nsteps > 0) {
+        // one synchronisation per call: the non-finite flag (and the step sizes if asked for)
+        if (dts_out) ARK_CUDA(cudaMemcpyAsync(dts_out, s->dtlog, (size_t)nsteps * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        ARK_CUDA(cudaMemcpyAsync(s->h_pinned, s->result + 3, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
         ARK_CUDA(cudaStreamSynchronize(s->stream));
-        for (int i = 0; i < nsteps; ++i)
-            if (!(dts_out[i] > 0.0) || std::isinf(dts_out[i]))
-                return fail(ARK_ENONFINITE, "ark_run: non-finite CFL rate at step %s%lld", "", (long long)i);
+        if (s->h_pinned[0] != 0.0) return fail(ARK_ENONFINITE, "ark_run: a maximum CFL rate was not finite and positive%s");
     }
     return ARK_OK;
 }
 
 int ark_diagnostics(ark_solver* s, double* out) {
     if (!s || !out) return fail(ARK_EINVAL, "ark_diagnostics: NULL argument%s");
+    ARK_ON_DEVICE(s);
     const long long n = (long long)s->P.nx * s->P.ny * s->P.nz;
     const int nb = grid_for(n, 256, DIAG_BLOCKS);
     double* part = s->scratch + (MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG);     // tail of the rate scratch (see ark_create)
@@ -567,6 +619,7 @@ int ark_diagnostics(ark_solver* s, double* out) {
 
 int ark_debug_get_padded(ark_solver* s, double* rho, double* rhou, double* rhov, double* rhow, double* E) {
     if (!s || !rho || !rhou || !rhov || !E || (s->P.ndim == 3 && !rhow)) return fail(ARK_EINVAL, "ark_debug_get_padded: NULL argument%s");
+    ARK_ON_DEVICE(s);
     int rc = launch_bc(s, s->U[s->cur]);
     if (rc != ARK_OK) return rc;
     double* dst[5] = {rho, rhou, rhov, s->P.ndim == 3 ? rhow : E, E};

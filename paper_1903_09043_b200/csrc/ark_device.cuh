@@ -173,26 +173,58 @@ ARK_DEV void ark_tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::
 ARK_DEV void ark_tm_st1(unsigned a, double v0) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(a), ARK_LO(v0), ARK_HI(v0) : "memory");
 }
+ARK_DEV void ark_tm_st2(unsigned a, double v0, double v1) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1) : "memory");
+}
+ARK_DEV void ark_tm_ld2(unsigned a, double& v0, double& v1) {
+    int l0, h0, l1, h1;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1) : "r"(a) : "memory");
+    v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1);
+}
+// ARK_TM_GRAN: doubles moved per tcgen05 instruction.  Wide transfers need their 2*GRAN registers contiguous, which
+// costs register-packing moves; narrow ones cost more tcgen05 instructions.
+#ifndef ARK_TM_GRAN
+#define ARK_TM_GRAN 8
+#endif
+#if ARK_TM_GRAN >= 4
 ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1),
                  ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3) : "memory");
 }
+#elif ARK_TM_GRAN == 2
+ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) { ark_tm_st2(a, v0, v1); ark_tm_st2(a + 4, v2, v3); }
+#else
+ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) { ark_tm_st1(a, v0); ark_tm_st1(a + 2, v1); ark_tm_st1(a + 4, v2); ark_tm_st1(a + 6, v3); }
+#endif
+#if ARK_TM_GRAN >= 8
 ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(a),
                  ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3), ARK_LO(v4), ARK_HI(v4),
                  ARK_LO(v5), ARK_HI(v5), ARK_LO(v6), ARK_HI(v6), ARK_LO(v7), ARK_HI(v7) : "memory");
 }
+#else
+ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
+    ark_tm_st4(a, v0, v1, v2, v3); ark_tm_st4(a + 8, v4, v5, v6, v7);
+}
+#endif
 ARK_DEV void ark_tm_ld1(unsigned a, double& v0) {
     int l0, h0;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(l0), "=r"(h0) : "r"(a) : "memory");
     v0 = __hiloint2double(h0, l0);
 }
+#if ARK_TM_GRAN >= 4
 ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) {
     int l0, h0, l1, h1, l2, h2, l3, h3;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                  : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3) : "r"(a) : "memory");
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
 }
+#elif ARK_TM_GRAN == 2
+ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) { ark_tm_ld2(a, v0, v1); ark_tm_ld2(a + 4, v2, v3); }
+#else
+ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) { ark_tm_ld1(a, v0); ark_tm_ld1(a + 2, v1); ark_tm_ld1(a + 4, v2); ark_tm_ld1(a + 6, v3); }
+#endif
+#if ARK_TM_GRAN >= 8
 ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
     int l0, h0, l1, h1, l2, h2, l3, h3, l4, h4, l5, h5, l6, h6, l7, h7;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -201,6 +233,11 @@ ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& 
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
     v4 = __hiloint2double(h4, l4); v5 = __hiloint2double(h5, l5); v6 = __hiloint2double(h6, l6); v7 = __hiloint2double(h7, l7);
 }
+#else
+ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
+    ark_tm_ld4(a, v0, v1, v2, v3); ark_tm_ld4(a + 8, v4, v5, v6, v7);
+}
+#endif
 #endif
 
 // ------------------------------------------------------------------------------------------------
@@ -368,7 +405,13 @@ ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
                 Tg = 2.0 * P.bcv[AXIS][side] - ws.T;
             }
             const double delta = (side == 0 ? -1.0 : 1.0) * P.g[AXIS] * P.h;
-            const double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
+            double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
+            // A9 needs T_g > |g_d| h / 2: otherwise relation (14) has no positive solution; flag the cell (NaN reaches the
+            // CFL reduction, which reports ARK_ENONFINITE) instead of marching on with a negative ghost density
+            // (only ghost cells that face interior cells: edge / corner ghosts mirror ghost cells of another wall and only
+            // their velocity is ever used, by the diagonal points of the viscous stencil)
+            const bool faces_interior = (AXIS == 0) || (c[0] >= 0 && c[0] < P.nx && (AXIS == 1 || (c[1] >= 0 && c[1] < P.ny)));
+            if (faces_interior && !(rg > 0.0)) rg = __longlong_as_double(0x7ff8000000000000LL);
             const double pg = rg * Tg;
             U[jg] = rg;
             U[P.fstride + jg] = rg * ug[0];
@@ -519,6 +562,8 @@ ARK_GLOBAL void ark_k_diag_pass2(const double* __restrict__ part, int nblocks, d
 // pass 2: single block over the per-block values; result[0] = max rate,
 // result[1] = dt = cfl / max rate (used by the device-side time loop of ark_run).  With dt_log the step size is also
 // appended at dt_log[*log_count] (a device-side counter, so that the launch can be replayed from a CUDA graph).
+// result[3] is a STICKY flag (never cleared here): set to 1.0 when a maximum rate was not finite and positive, so that a
+// device-side time loop (ark_run) can report a blown-up state without a host round trip per step (reading A15).
 ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, double cfl, double* __restrict__ result,
                                 double* __restrict__ dt_log, int* __restrict__ log_count) {
     ARK_SHARED double red[32];
@@ -528,6 +573,7 @@ ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, d
     if (threadIdx.x == 0) {
         result[0] = m;
         result[1] = cfl / m;
+        if (!(m > 0.0) || m > 1.7e308) result[3] = 1.0;
         if (dt_log) { const int i = *log_count; dt_log[i] = cfl / m; *log_count = i + 1; }
     }
 }

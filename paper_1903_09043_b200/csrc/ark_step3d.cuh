@@ -92,6 +92,8 @@ struct ArkMarch3 {
     int s, ca;                           // exchange slot (pair * RX + lane); UR column of row a (row b: + RX)
     int k0, k1;
     bool inU[2], want_rate;
+    int xwrap;                           // periodic x: offset of the ghost copy of this column (+nx, -nx) or 0
+    bool xwrap_any;                      // warp-uniform: some lane of the warp owns a column with a ghost copy
     int uq, un, unn, pc, pn;             // ring slots of planes q, q+1, q+2 (UR); q, q+1 (PB)
     // z pipelines of the two columns: the acoustic z face (q-1|q) stays in registers, everything else is parked in
     // TMEM between its uses (primitives of planes q-1 / q / q+1 in two alternating slots, U~(q-1), the running
@@ -562,6 +564,12 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
                         double* __restrict__ o = M.Ocur + r * M.px;          // plane q-1 of this column
                         o[0] = out[r][0]; o[M.fs] = out[r][1]; o[2 * M.fs] = out[r][2]; o[3 * M.fs] = out[r][3]; o[4 * M.fs] = out[r][4];
                     }
+                    if (M.xwrap_any && M.inU[r] && M.xwrap != 0) {
+                        // periodic x: the first / last two columns also fill the opposite ghost columns of the new
+                        // state, so that the next step needs no x ghost-fill launch
+                        double* __restrict__ o = M.Ocur + r * M.px + M.xwrap;
+                        o[0] = out[r][0]; o[M.fs] = out[r][1]; o[2 * M.fs] = out[r][2]; o[3 * M.fs] = out[r][3]; o[4 * M.fs] = out[r][4];
+                    }
                 }
                 if (M.want_rate) {
                     // CFL rate of the new state (reading A4), both rows in lock-step
@@ -754,6 +762,16 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     M.inU[0] = tile && inx && gja < P.ny;
     M.inU[1] = tile && inx && gja + 1 < P.ny;
     M.want_rate = rate_scratch != nullptr;
+    M.xwrap = 0;
+    if (P.bc[0][0] == ARK_BCK_PERIODIC && lane >= 2 && lane < 2 + TX) {
+        if (gi < 2) M.xwrap = P.nx;
+        else if (gi >= P.nx - 2 && gi < P.nx) M.xwrap = -P.nx;
+    }
+#ifndef ARK_HOST_EMU
+    M.xwrap_any = __any_sync(0xffffffffu, M.xwrap != 0);
+#else
+    M.xwrap_any = true;
+#endif
 
     const ArkStepConst K = ark_step_const(P, dt_value, dt_dev);
     M.pstride = (long long)P.px * P.py;

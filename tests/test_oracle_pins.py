@@ -672,3 +672,23 @@ def test_diagnostics_closed_forms():
     assert abs(d2["max_speed"] - s2) < 1e-14
     assert abs(d2["mean_speed"] - (speed * (nx * ny * nz - 1) + s2) / (nx * ny * nz)) < 1e-14
     assert abs(d2["max_mach"] - s2 / math.sqrt(gamma * p / rho)) < 1e-13 and abs(d2["mass"] - d["mass"]) < 1e-13
+
+
+def test_wall_closure_needs_a_positive_ghost_density():
+    """Reading A9: relation (14) gives rho_g = (p + rho delta / 2) / (T_g - delta / 2), which is only a
+    density when T_g > |g| h / 2.  Closed form on one column: with T_g below that bound the ghost cell is flagged
+    (NaN) and max_rate of the ghost-filled state is non-finite; just above it the ghost density is positive and obeys
+    relation (14) exactly."""
+    for T, ok in ((0.6, True), (0.4, False)):
+        prm = I.make_params(4, 4, 1, 1.0, 1.4, g=(0.0, -1.0, 0.0), bc_type=((PER, PER), (REF, REF), (0, 0)))
+        rho = np.full((1, 4, 4), 2.0)
+        p = rho * T
+        U = [rho, np.zeros_like(rho), np.zeros_like(rho), None, p / 0.4]
+        G = O.fill_ghosts(prm, U)
+        top = G[0][0, -2, 2:-2]                 # first ghost layer above the top wall: delta = Phi_prev - Phi_g = -|g| h
+        bot = G[0][0, 1, 2:-2]                  # first ghost layer below the bottom wall: delta = +|g| h
+        if ok:
+            assert np.allclose(top, (2.0 * T - 0.5 * 2.0) / (T + 0.5), rtol=1e-15) and (top > 0).all()
+            assert np.allclose(bot, (2.0 * T + 0.5 * 2.0) / (T - 0.5), rtol=1e-14) and (bot > 0).all()
+        else:
+            assert np.isnan(top).all() and np.isnan(bot).all()
