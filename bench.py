@@ -3,12 +3,19 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
 
-A "step" is one pass of the whole hot path over the synthetic workload: ghost fill (3 kernels), fused
-acoustic+transport+dissipative+update kernel with the CFL epilogue, the second reduction pass and the 16-byte
-device->host read of dt (ark_compute_dt) -- exactly the loop {dt = ark_compute_dt(cfl); ark_step(dt)}.
+A "step" is one pass of the whole hot path over the synthetic workload: ghost fill (y, z sweeps; the periodic x ghost
+columns are written by the step kernel itself), fused acoustic+transport+dissipative+update kernel with the CFL
+epilogue, the second reduction pass and the 16-byte device->host read of dt (ark_compute_dt) -- exactly the loop
+{dt = ark_compute_dt(cfl); ark_step(dt)}.
+
+The JSON line of the default workload (config5_512) also carries, under "also", the same measurement of the other
+roofline target of north_star (config4_256).  The fp64 peak of the "alu" roofline is MEASURED in the same run
+(ark_measure_fp64_peak: DFMA chains); the ncu-derived per-cell counters come from profiles/r02_step_kernel_counters.csv
+and are only reported when that file was captured for the kernel revision of the loaded library.
 
 Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs N independent
-replicas of the workload, one process per GPU (torchrun), no data-path collective; value = N * cells * K / max time.
+replicas of the workload, one process per GPU, no data-path collective; value = N * cells * K / max time.  Started
+without a torchrun environment, `--gpus N` (N > 1) re-launches itself under torch.distributed.run with N ranks.
 """
 import argparse
 import json
@@ -28,8 +35,8 @@ CFL = 0.4
 
 WORKLOADS = {
     # name: (builder name in inputs, n, bytes per cell update, oracle sample size)
-    "config5_512": ("config5_convection3d", 512, 80, 112),
-    "config4_256": ("config4_rb3d", 256, 80, 112),
+    "config5_512": ("config5_convection3d", 512, 80, 256),     # oracle sample: 256^3 (~6 s per step on one core)
+    "config4_256": ("config4_rb3d", 256, 80, 256),
     "config3_1024x512": ("config3_rb2d", (1024, 512), 64, (512, 256)),
     "config2_512": ("config2_gresho", 512, 64, 512),
     "config1_128": ("config1_atmosphere", 128, 64, 128),
@@ -48,14 +55,41 @@ def build_workload(name, device=None, sample=False):
     return prm, U, bpc
 
 
-# fp64 ALU roof: 64 fp64 instructions / clk / SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on
-# .peak_sustained = 64) x 148 SMs x clocks.max.sm 1965 MHz = 18.61 T fp64-instr/s (an FMA counts once).
+# fp64 ALU roof: measured in the same run by a register-resident DFMA-chain kernel of the library
+# (ark_measure_fp64_peak).  For context: 64 fp64 instructions / clk / SM x 148 SMs x 1965 MHz = 18.61 T instr/s nominal.
 FP64_INSTR_PER_CLK_SM, N_SM, SM_MAX_MHZ = 64, 148, 1965.0
-# fp64 thread-instructions per cell update of the step kernel (halo recomputation included), from the committed ncu
-# capture of each kernel variant (profiles/): sum of DADD+DMUL+DFMA+DSETP warp instructions x 32 / cells.
-FP64_INSTR_PER_CELL = {"config5_512": 430.6, "config4_256": 459.7}
-# dram__bytes_read.sum + dram__bytes_write.sum per step-kernel launch from the committed `ncu --set full` capture
-DRAM_TRAFFIC_BYTES = {"config5_512": 11400.4e6, "config4_256": 1423.8e6}
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02_step_kernel_counters.csv")
+
+
+def kernel_rev(version_string):
+    """'... kernels r2.1)' -> 'r2.1': the revision tag the ncu counters in profiles/ are recorded against."""
+    import re
+    m = re.search(r"kernels ([^\s)]+)\)", version_string)
+    return m.group(1) if m else None
+
+
+def load_counters(path=COUNTERS_CSV):
+    """workload -> {kernel_rev, fp64_instr_per_cell, dram_bytes_per_launch, source}: per-cell fp64 thread-instructions
+    (DADD+DMUL+DFMA+DSETP warp instructions x 32 / cells, halo recomputation included) and dram__bytes_read.sum +
+    dram__bytes_write.sum per step-kernel launch, from the committed `ncu --set full` captures."""
+    import csv
+    out = {}
+    try:
+        with open(path) as fh:
+            for row in csv.DictReader(r for r in fh if not r.startswith("#")):
+                out[row["workload"]] = {"kernel_rev": row["kernel_rev"], "fp64_instr_per_cell": float(row["fp64_instr_per_cell"]),
+                                        "dram_bytes_per_launch": float(row["dram_bytes_per_launch"]), "source": row["source"]}
+    except OSError:
+        pass
+    return out
+
+
+def counters_for(workload, version_string, table=None):
+    """The counters of `workload` if they were captured for the loaded library's kernel revision, else None (stale)."""
+    c = (load_counters() if table is None else table).get(workload)
+    if c is None or c["kernel_rev"] != kernel_rev(version_string):
+        return None
+    return c
 
 
 def max_over_ranks(x, dist=None, device=None):
@@ -74,16 +108,19 @@ def whole_job_value(world, ncell, steps, seconds):
     return world * ncell * steps / seconds
 
 
-def fp64_roofline(workload, ncell, kern_ms):
-    """The viscous 3D step is fp64-ALU-bound before it is HBM-bound: second roofline object."""
-    ipc = FP64_INSTR_PER_CELL.get(workload)
-    if ipc is None:
+def fp64_roofline(counters, ncell, kern_ms, peak=None, peak_source=None):
+    """The viscous 3D step is fp64-ALU-bound before it is HBM-bound: second roofline object.
+    counters: counters_for(...) or None; peak in 1e12 fp64 thread-instructions/s (measured) or None (nominal)."""
+    if counters is None:
         return None
-    peak = FP64_INSTR_PER_CLK_SM * N_SM * SM_MAX_MHZ * 1e6 / 1e12
+    if peak is None:
+        peak = FP64_INSTR_PER_CLK_SM * N_SM * SM_MAX_MHZ * 1e6 / 1e12
+        peak_source = "nominal: 64 fp64 instr/clk/SM x 148 SMs x 1965 MHz"
+    ipc = counters["fp64_instr_per_cell"]
     achieved = ipc * ncell / (kern_ms * 1e-3) / 1e12
-    return {"bound": "alu", "kernel": "ark_k_step", "achieved": achieved, "peak": peak, "unit": "T fp64-instr/s",
-            "frac": achieved / peak, "fp64_instr_per_cell": ipc,
-            "peak_source": "derived: 64 fp64 instr/clk/SM (ncu peak_sustained) x 148 SMs x 1965 MHz"}
+    return {"bound": "alu", "kernel": "ark_k_step3", "achieved": achieved, "peak": peak, "unit": "T fp64-instr/s",
+            "frac": achieved / peak, "fp64_instr_per_cell": ipc, "peak_source": peak_source,
+            "counters_from": counters["source"], "kernel_rev": counters["kernel_rev"]}
 
 
 def measured_peaks():
@@ -143,6 +180,20 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def host_cpu():
+    """(logical CPUs of the box, CPU model string) for the cpu_baseline record."""
+    model = None
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for ln in fh:
+                if ln.lower().startswith("model name"):
+                    model = ln.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return os.cpu_count(), model
+
+
 def oracle_timed(name, steps, warmup):
     """The oracle as it stands, single thread, on a bounded sample of the workload (same recipe, smaller grid)."""
     from oracle import ark_oracle as O
@@ -161,52 +212,44 @@ def oracle_timed(name, steps, warmup):
     return ncell * steps / el, el / steps * 1e3, sample
 
 
+def cpu_baseline_record(val, sample):
+    nproc, model = host_cpu()
+    return {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "host_nproc": nproc, "host_cpu": model}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    k = max(1, min(args.steps, 5))
-    val, ms, sample = oracle_timed(args.workload, k, 1)
+    k = max(1, min(args.steps, 4))
+    val, ms, sample = oracle_timed(args.workload, k, 0)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": k,
-            "warmup": 1, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "warmup": 0, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "note": "oracle (oracle/ark_oracle.cpp) on host cores; each step is a bounded sample: " + sample},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": cpu_baseline_record(val, sample),
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
-def run_ours(args):
+def measure_workload(name, K, W, dev, local, world, dist, e2e=True):
+    """K timed steps of {compute_dt; step} of one workload (after W warm-up steps), device-timed on the solver's
+    stream, max over ranks; the step kernel's own time from events the library records around its launches; optionally
+    the end-to-end variant with HOST buffers.  Returns a dict of raw numbers."""
     import torch
     from paper_1903_09043_b200 import binding
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    binding.load()
-    prm, U, bpc = build_workload(args.workload, device=dev)
+    prm, U, bpc = build_workload(name, device=dev)
     U = [None if a is None else a.reshape(-1).contiguous() for a in U]
     ncell = prm["nx"] * prm["ny"] * prm["nz"]
     s = binding.Solver(prm, device=dev)
     s.set_state(U)
-
-    W = max(args.warmup, 3)
-    K = args.steps
     for _ in range(W):
         s.step(s.compute_dt(CFL))
     torch.cuda.synchronize()
@@ -229,62 +272,122 @@ def run_ours(args):
     s.step_kernel_timing(False)
     launches = s.launch_count() - l0
     ms_total = max_over_ranks(ms_total, dist, dev)
-    value = whole_job_value(world, ncell, K, ms_total * 1e-3)
+    out = {"prm": prm, "bpc": bpc, "ncell": ncell, "ms_total": ms_total, "kern_ms": kern_ms, "kern_n": kern_n,
+           "launches": launches, "clocks": clocks, "value": whole_job_value(world, ncell, K, ms_total * 1e-3)}
 
     # sanity: state still finite after the timed steps
-    dt_chk = s.compute_dt(CFL)
-    assert dt_chk > 0
+    assert s.compute_dt(CFL) > 0
 
-    # ---- end to end through the C ABI with HOST buffers (pinned): set_state_host + compute_dt + step + get_state_host
-    e2e_steps = max(1, min(K, 3))
-    host_in = [None if a is None else a.cpu().pin_memory() for a in U]
-    host_out = [None if a is None else torch.empty_like(a) .pin_memory() for a in host_in]
-    nfield = sum(a is not None for a in host_in)
-    s.set_state_host(host_in)
-    s.step(s.compute_dt(CFL))
-    s.get_state_host(host_out)                      # warm-up of the e2e path
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    if e2e:
+        # ---- end to end through the C ABI with HOST buffers (pinned): set_state_host + compute_dt + step + get_state_host
+        e2e_steps = max(1, min(K, 3))
+        host_in = [None if a is None else a.cpu().pin_memory() for a in U]
+        host_out = [None if a is None else torch.empty_like(a) .pin_memory() for a in host_in]
+        nfield = sum(a is not None for a in host_in)
         s.set_state_host(host_in)
         s.step(s.compute_dt(CFL))
-        s.get_state_host(host_out)
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = max_over_ranks(e2e_s, dist, dev)
-    e2e_val = whole_job_value(world, ncell, e2e_steps, e2e_s)
+        s.get_state_host(host_out)                      # warm-up of the e2e path
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            s.set_state_host(host_in)
+            s.step(s.compute_dt(CFL))
+            s.get_state_host(host_out)
+        torch.cuda.synchronize()
+        e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
+        out["e2e"] = {"value": whole_job_value(world, ncell, e2e_steps, e2e_s), "unit": UNIT,
+                      "h2d_bytes_per_step": nfield * ncell * 8, "d2h_bytes_per_step": nfield * ncell * 8 + 16, "steps": e2e_steps,
+                      "path": "ark_set_state_host + ark_compute_dt + ark_step + ark_get_state_host, pinned host buffers"}
+    s.close()
+    del s, U
+    torch.cuda.empty_cache()
+    return out
+
+
+def roofline_objects(name, m, world, version, fp64_peak):
+    """(hbm roofline, fp64 roofline) of one measured workload."""
+    peak, peak_src = measured_peaks()
+    alg_bytes = m["bpc"] * m["ncell"]                 # per launch of the dominant (fused step) kernel
+    kern_avg_ms = m["kern_ms"] / max(m["kern_n"], 1)
+    achieved = alg_bytes / (kern_avg_ms * 1e-3) / 1e9
+    c = counters_for(name, version)
+    hbm = {"bound": "hbm", "kernel": "ark_k_step3" if m["prm"]["nz"] > 1 else "ark_k_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
+           "frac": achieved / peak, "traffic": c["dram_bytes_per_launch"] if c else None,
+           "traffic_from": c["source"] if c else "no ncu capture of kernel revision %s in profiles/" % kernel_rev(version),
+           "peak_source": peak_src, "algorithmic_bytes_per_cell": m["bpc"], "kernel_ms": kern_avg_ms,
+           "kernel_launches_timed": m["kern_n"], "kernel_share_of_step": m["kern_ms"] / m["ms_total"],
+           "effective_whole_step_frac": m["bpc"] * m["value"] / world / 1e9 / peak}
+    alu = fp64_roofline(c, m["ncell"], kern_avg_ms, fp64_peak,
+                        "measured in this run (ark_measure_fp64_peak: register-resident DFMA chains; nominal 18.61)" if fp64_peak else None)
+    return hbm, alu
+
+
+def run_ours(args):
+    import torch
+    from paper_1903_09043_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    binding.load()
+    version = binding.version_string()
+    W = max(args.warmup, 3)
+    K = args.steps
+    m = measure_workload(args.workload, K, W, dev, local, world, dist)
+    fp64_peak = binding.measure_fp64_peak()
+    also = None
+    if args.workload == "config5_512" and not args.no_also:
+        # the other roofline target of north_star, same measurement, in the same driver-run line
+        also = ("config4_256", measure_workload("config4_256", max(K, 20), W, dev, local, world, dist, e2e=False))
 
     if rank == 0:
-        peak, peak_src = measured_peaks()
-        alg_bytes = bpc * ncell                       # per launch of the dominant (fused step) kernel
-        kern_avg_ms = kern_ms / max(kern_n, 1)
-        achieved = alg_bytes / (kern_avg_ms * 1e-3) / 1e9
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        prm, bpc, ncell = m["prm"], m["bpc"], m["ncell"]
+        hbm, alu = roofline_objects(args.workload, m, world, version, fp64_peak)
+        line = {"metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": m["ms_total"] / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": args.workload, "grid": [prm["nx"], prm["ny"], prm["nz"]], "cfl": CFL,
-                           "step": "ark_compute_dt + ark_step (ghost fill x/y/z, fused step kernel, CFL pass 2, 16 B D2H)",
+                           "step": "ark_compute_dt + ark_step (ghost fill y/z, fused step kernel incl. periodic x ghosts, CFL pass 2, 16 B D2H)",
                            "l2": "inputs larger than L2 (state %.2f GB)" % (bpc / 2 * ncell / 1e9) if bpc / 2 * ncell > 200e6
                                  else "state fits in L2 (%.1f MB): latency-bound config, HBM roofline not meaningful" % (bpc / 2 * ncell / 1e6),
                            "parallelism": "replicas only" if world > 1 else "single GPU",
-                           "library": binding.version_string()},
-                "roofline": {"bound": "hbm", "kernel": "ark_k_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                             "frac": achieved / peak, "traffic": DRAM_TRAFFIC_BYTES.get(args.workload), "peak_source": peak_src,
-                             "algorithmic_bytes_per_cell": bpc, "kernel_ms": kern_avg_ms, "kernel_launches_timed": kern_n,
-                             "kernel_share_of_step": kern_ms / ms_total,
-                             "effective_whole_step_frac": bpc * value / world / 1e9 / peak},
-                "roofline_fp64": fp64_roofline(args.workload, ncell, kern_avg_ms),
-                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": nfield * ncell * 8,
-                        "d2h_bytes_per_step": nfield * ncell * 8 + 16, "steps": e2e_steps,
-                        "path": "ark_set_state_host + ark_compute_dt + ark_step + ark_get_state_host, pinned host buffers"},
-                "gpu_launches": launches, "clocks": clocks}
+                           "library": version},
+                "roofline": hbm, "roofline_fp64": alu, "e2e": m["e2e"], "gpu_launches": m["launches"], "clocks": m["clocks"]}
+        if also is not None:
+            name2, m2 = also
+            hbm2, alu2 = roofline_objects(name2, m2, world, version, fp64_peak)
+            k2 = m2["kern_n"]
+            line["also"] = {"workload": name2, "grid": [m2["prm"]["nx"], m2["prm"]["ny"], m2["prm"]["nz"]], "steps": k2,
+                            "value": m2["value"], "unit": UNIT, "ms_per_step": m2["ms_total"] / k2, "roofline": hbm2,
+                            "roofline_fp64": alu2, "gpu_launches": m2["launches"], "clocks": m2["clocks"]}
         if world == 1 and not args.no_cpu_baseline:
-            val, ms, sample = oracle_timed(args.workload, 3, 1)
-            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+            val, ms, sample = oracle_timed(args.workload, 2, 0)
+            line["cpu_baseline"] = cpu_baseline_record(val, sample)
         print(json.dumps(line))
-    s.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a torchrun environment: re-launch under torch.distributed.run, one rank per GPU
+    (the launch line the driver itself uses), and pass its output through."""
+    import socket
+    sk = socket.socket()
+    sk.bind(("127.0.0.1", 0))
+    port = sk.getsockname()[1]
+    sk.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -295,9 +398,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5_512", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the config4_256 measurement that rides along with config5_512")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))
     else:
         run_ours(args)
 

@@ -112,6 +112,12 @@ int ark_debug_get_padded(ark_solver*, double* rho, double* rhou, double* rhov, d
 int ark_step_kernel_timing(ark_solver*, int enable);
 int ark_step_kernel_time(ark_solver*, double* total_ms, int* launches);
 
+/* Measurement support (no handle): runs a register-resident DFMA-chain kernel on the current device and returns the
+ * sustained fp64 instruction rate in 1e12 thread-instructions per second (one DFMA = one instruction).  bench.py
+ * reports the "alu" roofline of the fp64-bound step kernel against it (the fp64 peak must be measured,
+ * not derived).  Synchronises the stream. */
+int ark_measure_fp64_peak(double* tinstr_per_s, void* cuda_stream);
+
 /* Number of kernels this library has launched on behalf of the handle since creation. */
 long long ark_launch_count(const ark_solver*);
 

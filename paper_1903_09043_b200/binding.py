@@ -17,7 +17,7 @@ BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
            "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_diagnostics", "ark_debug_get_padded",
-           "ark_step_kernel_timing", "ark_step_kernel_time", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
+           "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
 
 
 class ark_bc(C.Structure):
@@ -63,6 +63,8 @@ def load():
     lib.ark_step_kernel_timing.restype = ip
     lib.ark_step_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     lib.ark_step_kernel_time.restype = ip
+    lib.ark_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), vp]
+    lib.ark_measure_fp64_peak.restype = ip
     lib.ark_launch_count.argtypes = [vp]
     lib.ark_launch_count.restype = C.c_longlong
     lib.ark_destroy.argtypes = [vp]
@@ -75,6 +77,13 @@ def load():
 
 def version_string():
     return load().ark_version_string().decode()
+
+
+def measure_fp64_peak():
+    """Sustained fp64 instruction rate of the current device in 1e12 thread-instructions/s (DFMA chains)."""
+    out = C.c_double(0.0)
+    _check(load().ark_measure_fp64_peak(C.byref(out), C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+    return out.value
 
 
 def workspace_bytes(nx, ny, nz):

@@ -30,6 +30,7 @@ constexpr int TX3 = ARK_TX3, NW3 = ARK_NW3;   // 3D: outputs per row, row pairs 
 constexpr int TY3 = 2 * NW3 - 4;
 constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
 
+#define ARK_KERNEL_REV "r2.1"
 constexpr int CFL_BLOCK = 256;
 #define ARK_MAX_TIMED 4096
 constexpr int MAX_SCRATCH = 1 << 16;          // per-block rate slots
@@ -262,8 +263,10 @@ const char* ark_last_error(void) { return g_err; }
 
 const char* ark_version_string(void) {
     static char buf[256];
-    snprintf(buf, sizeof buf, "ark-b200 0.1 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d (%d row pairs) tile2d=%dx%d)", ARK_K_IMPEDANCE, ARK_NG,
-             TX3, TY3, NW3, TX2, TY2);
+    // ARK_KERNEL_REV names the revision of the step kernels the committed ncu counters (profiles/) belong to: bump it
+    // with every change to the kernels' arithmetic or memory traffic
+    snprintf(buf, sizeof buf, "ark-b200 0.2 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d (%d row pairs) tile2d=%dx%d; kernels %s)", ARK_K_IMPEDANCE, ARK_NG,
+             TX3, TY3, NW3, TX2, TY2, ARK_KERNEL_REV);
     return buf;
 }
 
@@ -614,6 +617,35 @@ int ark_diagnostics(ark_solver* s, double* out) {
     out[3] = h[3];                 // max Mach number
     out[4] = h[4] * vol;           // mass
     out[5] = h[5] * vol;           // total energy incl. potential
+    return ARK_OK;
+}
+
+int ark_measure_fp64_peak(double* tinstr_per_s, void* cuda_stream) {
+    if (!tinstr_per_s) return fail(ARK_EINVAL, "ark_measure_fp64_peak: NULL argument%s");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    ARK_CUDA(cudaGetDevice(&dev));
+    ARK_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    double* sink = nullptr;
+    ARK_CUDA(cudaMalloc((void**)&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    ARK_CUDA(cudaEventCreate(&e0));
+    ARK_CUDA(cudaEventCreate(&e1));
+    const int threads = 512, blocks = nsm * 2, iters = 4096;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {          // the first repetition warms up
+        ARK_CUDA(cudaEventRecord(e0, st));
+        ark_k_dfma_peak<<<blocks, threads, 0, st>>>(sink, iters, 0.999999, 1e-7);
+        ARK_CUDA(cudaEventRecord(e1, st));
+        ARK_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        ARK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        const double rate = (double)blocks * threads * (double)iters * 64.0 / (ms * 1e-3) / 1e12;
+        if (rep > 0 && rate > best) best = rate;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    ARK_CUDA(cudaGetLastError());
+    *tinstr_per_s = best;
     return ARK_OK;
 }
 

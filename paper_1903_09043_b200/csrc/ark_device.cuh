@@ -577,3 +577,22 @@ ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, d
         if (dt_log) { const int i = *log_count; dt_log[i] = cfl / m; *log_count = i + 1; }
     }
 }
+
+// ------------------------------------------------------------------------------------------------
+// fp64 pipe microbenchmark (measurement support for the "alu" roofline of bench.py): register-resident DFMA chains,
+// 8 independent chains per thread, no memory traffic.  One DFMA = one fp64 instruction (SURVEY 8(d) asks for a
+// MEASURED fp64 peak next to the measured HBM peak).
+// ------------------------------------------------------------------------------------------------
+ARK_GLOBAL void ark_k_dfma_peak(double* __restrict__ sink, int iters, double a, double b) {
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1.0, x2 = x0 + 2.0, x3 = x0 + 3.0, x4 = x0 + 4.0, x5 = x0 + 5.0, x6 = x0 + 6.0, x7 = x0 + 7.0;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    const double r = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (r == 123.456) sink[0] = r;             // never true for the arguments used; keeps the chains alive
+}
+

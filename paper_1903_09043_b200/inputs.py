@@ -264,6 +264,60 @@ def config5_convection3d(n=512, seed=1005, amp=1e-2, theta=1, device=None, box=N
     return _convection3d(n, n, 1.0, 100.0, 1.0e-4, 2.5e-4, BC_REFLECTING, amp, seed, theta, device, box, heat=heat)
 
 
+# --------------------------------------------------------------------------- second workloads
+def rayleigh_taylor(nx=200, ny=600, C=0.01, theta=1, mu=0.0, device=None):
+    """Rayleigh-Taylor test case: domain [-0.25,0.25] x [-0.75,0.75] (L_x = 0.5, L_y = 1.5), rho = 1
+    for y < 0 and 2 for y >= 0, u = 0, v = C/4 (1 + cos(2 pi x / L_x)) (1 + cos(2 pi y / L_y)), C = 0.01, resolution
+    200 x 600.  The printed pressure "p = rho g y" is an abbreviation (it would be negative on one side): reading A23
+    takes the classical setup p = p0 + rho g_y y with g = (0, -0.1), p0 = 2.5, gamma = 1.4, periodic x, reflecting y
+    walls, for which the C = 0 state satisfies the discrete balance (14) exactly, as PAPER.md:421 states."""
+    if ny * 0.5 / nx != 1.5:
+        raise ValueError("rayleigh_taylor: the domain is 0.5 x 1.5, so ny must be 3 nx")
+    h = 0.5 / nx
+    gamma, gy, p0 = 1.4, -0.1, 2.5
+    x = -0.25 + (np.arange(nx) + 0.5) * h
+    y = -0.75 + (np.arange(ny) + 0.5) * h
+    rho_c = np.where(y < 0.0, 1.0, 2.0)
+    p_c = p0 + rho_c * gy * y
+    rho = _full(_col(rho_c, 1, device), nx, ny, 1, device)
+    p = _full(_col(p_c, 1, device), nx, ny, 1, device)
+    vx = _col(1.0 + np.cos(2.0 * np.pi * x / 0.5), 0, device)
+    vy = _col(1.0 + np.cos(2.0 * np.pi * y / 1.5), 1, device)
+    v = _full((0.25 * C) * vx * vy, nx, ny, 1, device)
+    zero = rho * 0.0
+    E = _energy(gamma, rho, zero, v, None, p)
+    prm = make_params(nx, ny, 1, h, gamma, g=(0.0, gy, 0.0), mu=mu, theta=theta,
+                      bc_type=((BC_PERIODIC, BC_PERIODIC), (BC_REFLECTING, BC_REFLECTING), (0, 0)))
+    return prm, [rho, zero, rho * v, None, E]
+
+
+def rb2d_chi21(nx=128, ny=128, seed=1021, amp=1e-4, theta=1, ra_over_rac=10.0, device=None):
+    """Strongly stratified 2D Rayleigh-Benard case: density ratio chi = 21 across the layer (m = 1.3,
+    gamma = 5/3, g = (0,-1)), polytrope initialised by recursion (14), the temperature flux imposed on the
+    bottom boundary (here the conductive flux kappa beta of the polytrope, so the unperturbed state is
+    steady), fixed temperature at the top, periodic x.  mu, kappa from a mid-layer Rayleigh number ra_over_rac x 1707.76
+    at Pr = 1 (the paper prints none: workload parameters)."""
+    h = 1.0 / ny
+    gamma = 5.0 / 3.0
+    m, chi = 1.3, 21.0
+    beta = 1.0 / (m + 1.0)
+    T_top = beta / (chi ** (1.0 / m) - 1.0)
+    T_bot = T_top + beta
+    Tc, rho_c = polytrope(ny, h, T_top, beta, m)
+    rho_mid = ((0.5 * (T_top + T_bot)) / T_top) ** m
+    mu, kappa = _rb_mu_kappa(gamma, m, T_top, T_bot, rho_mid, ra_over_rac * 1707.76, 1.0)
+    rho = _full(_col(rho_c, 1, device), nx, ny, 1, device)
+    T = _full(_col(Tc, 1, device), nx, ny, 1, device)
+    if amp != 0.0:
+        T = T * (1.0 + amp * _noise(seed, nx, ny, 1, 1, 0, device))
+    p = rho * T
+    zero = rho * 0.0
+    prm = make_params(nx, ny, 1, h, gamma, g=(0.0, -1.0, 0.0), mu=mu, kappa=kappa, theta=theta,
+                      bc_type=((BC_PERIODIC, BC_PERIODIC), (BC_FLUX, BC_FIXED_T), (0, 0)),
+                      bc_value=((0, 0), (kappa * beta, T_top), (0, 0)))
+    return prm, [rho, zero, zero.clone() if device is not None else zero.copy(), None, p / (gamma - 1.0)]
+
+
 # --------------------------------------------------------------------------- extra test problems
 def sod_tube(nx=100, ny=4, theta=1):
     """Sod shock tube along x on [0,1], reflecting x walls, periodic y (reading A16)."""

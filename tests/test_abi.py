@@ -21,7 +21,7 @@ def test_exports_every_symbol_declared_in_header(lib):
     from paper_1903_09043_b200 import binding
     hdr = open(os.path.join(ROOT, "include", "ark.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = sorted(set(re.findall(r"\b(ark_[a-z_]+)\s*\(", hdr)))
+    declared = sorted(set(re.findall(r"\b(ark_[a-z0-9_]+)\s*\(", hdr)))
     assert declared, "no declarations found"
     for name in declared:
         assert hasattr(lib, name), name

@@ -1,6 +1,7 @@
 """Seeded input generators (paper_1903_09043_b200/inputs.py): determinism, numpy/torch agreement, per-cell
 regeneration of sub-boxes, and the discrete hydrostatic relation (14) of the initial columns."""
 import numpy as np
+import pytest
 import torch
 
 from paper_1903_09043_b200 import inputs as I
@@ -58,3 +59,27 @@ def test_columns_satisfy_discrete_hydrostatic_relation():
     assert abs(prm["mu"] - 7.473e-4) < 2e-6 and abs(prm["kappa"] - 1.8683e-3) < 5e-6
     prm, U = I.config3_rb2d(16, 8)
     assert abs(prm["mu"] - 1.8544e-3) < 2e-6 and abs(prm["kappa"] - 4.6361e-3) < 5e-6
+
+
+def test_second_workloads_follow_the_paper():
+    """Rayleigh-Taylor and the chi = 21 layer."""
+    prm, U = I.rayleigh_taylor(20, 60)
+    assert (prm["nx"], prm["ny"], prm["nz"]) == (20, 60, 1) and abs(prm["dx"] - 0.5 / 20) < 1e-16
+    rho = U[0][0]
+    assert (rho[:30] == 1.0).all() and (rho[30:] == 2.0).all()                 # rho = 1 for y < 0, 2 for y >= 0
+    v = U[2][0] / rho
+    assert abs(v.max() - 0.01 * np.cos(np.pi * 0.5 / 20) ** 2 * np.cos(np.pi * 0.5 / 60) ** 2) < 1e-12   # C/4 (1+cos)(1+cos) near the centre
+    assert v.min() >= 0.0 and np.abs(U[1]).max() == 0.0
+    p = 0.4 * (U[4][0] - 0.5 * rho * v * v)
+    h = prm["dx"]
+    lhs = p[1:, 0] - p[:-1, 0]                                                  # discrete balance (14) holds on every face
+    rhs = -0.5 * (rho[1:, 0] + rho[:-1, 0]) * 0.1 * h
+    assert np.abs(lhs - rhs).max() < 1e-15
+    with pytest.raises(ValueError):
+        I.rayleigh_taylor(20, 50)
+    prm, U = I.rb2d_chi21(16, 64)
+    assert prm["bc_type"][1] == (I.BC_FLUX, I.BC_FIXED_T)
+    beta = 1.0 / 2.3
+    assert abs(prm["bc_value"][1][0] - prm["kappa"] * beta) < 1e-16           # the polytrope's own conductive flux
+    T_top = prm["bc_value"][1][1]
+    assert abs(((T_top + beta) / T_top) ** 1.3 - 21.0) < 1e-10                 # chi = 21 wall to wall

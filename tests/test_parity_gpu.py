@@ -96,6 +96,10 @@ CONFIGS = {
     # (n = 64 keeps the top wall's ghost temperature above g h / 2, the precondition of reading A9; at n = 48 the
     # hydrostatic extrapolation has no positive ghost density, which both sides now flag as non-finite)
     "config5_mach_half_noise_64": lambda: I.config5_convection3d(64, amp=0.05),
+    # second workloads: Rayleigh-Taylor and the chi = 21 convection layer (:447)
+    "rayleigh_taylor_60x180": lambda: I.rayleigh_taylor(60, 180),
+    "rayleigh_taylor_theta_off_40x120": lambda: I.rayleigh_taylor(40, 120, theta=0),
+    "rb2d_chi21_96x80": lambda: I.rb2d_chi21(96, 80),
 }
 
 
@@ -485,3 +489,35 @@ def test_3d_baseline_configs_full_step_counts(B):
     assert abs(d1["mass"] - d0["mass"]) < 1e-12 * d0["mass"]
     gain = d1["total_energy"] - d0["total_energy"]
     assert abs(gain - F * 1.0 * sum(dts)) < 2e-12 * abs(d0["total_energy"]), (gain, F * sum(dts), d0["total_energy"])
+
+
+def test_second_workloads_at_full_size(B):
+    """Rayleigh-Taylor at the paper's 200 x 600 through the device-side loop: without perturbation the
+    two-layer state stays at rest; with it mass is conserved to round-off, the kinetic energy stays of the order of the
+    seeded perturbation over the first acoustic transient (2000 steps are t = 0.5, a third of a growth time) and the flow
+    stays far below Mach 1.  The chi = 21 layer at 256 x 256 stays at rest when unperturbed."""
+    prm, U = I.rayleigh_taylor(200, 600, C=0.0)
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    s.run(500, 0.4)
+    d = s.diagnostics()
+    s.close()
+    assert d["max_speed"] < 1e-12, d
+    prm, U = I.rayleigh_taylor(200, 600)
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    d0 = s.diagnostics()
+    s.run(2000, 0.4)
+    d1 = s.diagnostics()
+    s.close()
+    assert abs(d1["mass"] - d0["mass"]) <= 1e-12 * d0["mass"]             # mass
+    assert 0.05 * d0["kinetic_energy"] < d1["kinetic_energy"] < 2.0 * d0["kinetic_energy"]
+    assert np.isfinite(d1["max_mach"]) and d1["max_mach"] < 0.1              # max Mach
+    prm, U = I.rb2d_chi21(256, 256, amp=0.0)
+    s = B.Solver(prm)
+    s.set_state(to_dev(U))
+    s.run(1000, 0.4)
+    d = s.diagnostics()
+    s.close()
+    assert d["max_speed"] < 1e-12, d
+
