@@ -55,6 +55,8 @@ struct Cfg {
     int theta;       // 0: theta == 1 ; 1: eq. (13)
     int bc[3][2];    // [axis][lo,hi]
     double bcv[3][2];// wall temperature for BC_FIXED_T; heat flux entering the domain for BC_FLUX
+    const double* phi; // optional gravitational potential at the interior cell centres (dense, x fastest; PAPER.md:55 general
+                     // Phi(x)); NULL: Phi = -g.x with the constant vector g (reading A12).  Not owned.
 };
 
 struct Grid {
@@ -135,7 +137,44 @@ Face acoustic_face(double rhoL, double unL, double pL, double cL,
 // 1. ghost fill (reading A9).  Axis order x, y, z; each later axis sweeps the
 //    already-extended range of the earlier ones so edges and corners are set.
 // ---------------------------------------------------------------------------
-void fill_ghosts(const Cfg& cfg, const Grid& G, State& U) {
+// Padded potential for a run with an array-valued Phi (PAPER.md:55, :152 'Phi_{i+1} - Phi_i'): interior values from
+// cfg.phi; ghost values (reading A25): periodic axes wrap, wall axes continue Phi linearly from the two cells next to
+// the wall (Phi(-l) = Phi(0) + l (Phi(0) - Phi(1))), which reproduces a constant gravity exactly.  Same x, y, z sweep
+// order over already-extended ranges as the state's ghost fill.  Empty when cfg.phi == NULL (constant g).
+std::vector<double> padded_potential(const Cfg& cfg, const Grid& G) {
+    std::vector<double> P;
+    if (!cfg.phi) return P;
+    P.assign(G.ncell, 0.0);
+    size_t s = 0;
+    for (int k = 0; k < G.n[2]; ++k) for (int j = 0; j < G.n[1]; ++j) for (int i = 0; i < G.n[0]; ++i, ++s) P[G.at(i, j, k)] = cfg.phi[s];
+    for (int d = 0; d < cfg.ndim; ++d) {
+        int lo[3], hi[3];
+        for (int e = 0; e < 3; ++e) {
+            if (e < d && e < cfg.ndim) { lo[e] = -NG; hi[e] = G.n[e] + NG; }
+            else                       { lo[e] = 0;   hi[e] = G.n[e]; }
+        }
+        lo[d] = 0; hi[d] = 1;
+        const int n = G.n[d];
+        int c[3];
+        for (c[2] = lo[2]; c[2] < hi[2]; ++c[2])
+        for (c[1] = lo[1]; c[1] < hi[1]; ++c[1])
+        for (c[0] = lo[0]; c[0] < hi[0]; ++c[0]) {
+            auto at = [&](int i) { int q[3] = {c[0], c[1], c[2]}; q[d] = i; return G.at(q); };
+            for (int l = 1; l <= NG; ++l) {
+                if (cfg.bc[d][0] == BC_PERIODIC) {
+                    P[at(-l)] = P[at(n - l)];
+                    P[at(n - 1 + l)] = P[at(l - 1)];
+                } else {
+                    P[at(-l)] = P[at(0)] + l * (P[at(0)] - P[at(1)]);
+                    P[at(n - 1 + l)] = P[at(n - 1)] + l * (P[at(n - 1)] - P[at(n - 2)]);
+                }
+            }
+        }
+    }
+    return P;
+}
+
+void fill_ghosts(const Cfg& cfg, const Grid& G, State& U, const std::vector<double>& PhiP) {
     for (int d = 0; d < cfg.ndim; ++d) {
         int lo[3], hi[3];
         for (int e = 0; e < 3; ++e) {
@@ -180,8 +219,8 @@ void fill_ghosts(const Cfg& cfg, const Grid& G, State& U) {
                         for (int e = 0; e < 3; ++e) ug[e] = -ws.u[e];
                         Tg = 2.0 * cfg.bcv[d][side] - ws.T;
                     }
-                    // delta = Phi_prev - Phi_ghost, Phi = -g.x
-                    const double delta = (side == 0 ? -1.0 : 1.0) * cfg.g[d] * cfg.h;
+                    // delta = Phi_prev - Phi_ghost, Phi = -g.x (or the given potential)
+                    const double delta = PhiP.empty() ? (side == 0 ? -1.0 : 1.0) * cfg.g[d] * cfg.h : PhiP[jp] - PhiP[jg];
                     // eq. (14) with p_g = rho_g T_g:  rho_g = (p_prev + 1/2 rho_prev delta)/(T_g - 1/2 delta)
                     double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
                     // reading A9 requires T_g > |g_d| h / 2; without it relation (14) has no positive solution and the
@@ -256,10 +295,17 @@ void dissipative_face(const Cfg& cfg, const Grid& G, const Prim& W, int d, size_
 // eq. (11) literally with rho*calE = rho*E + rho*Phi,
 // Phi = -g.x at cell centres, converted back by the relaxation Psi = Phi
 // (PAPER.md:178).  The two agree to round-off (pin P4).
+// form == 2: the non-conservative energy scheme of Appendix B: the same mass and momentum updates;
+// the energy gets the source (dt/dx) (uS)_i, (uS)_i = 1/2 (u*_{i+1/2} S_{i+1/2} + u*_{i-1/2} S_{i-1/2}), instead of
+// the mass-flux-weighted gravity work.  Reading A24: the source belongs to the acoustic sub-step (the acoustic
+// energy equation of App. B carries -rho u . grad Phi), so (rho E)~ = (rho E - lam [Pi* u*] + lam (uS)_i) / L~, exactly as
+// (rho u)~ carries lam S_i; summing the two sub-steps gives the update printed at PAPER.md:538.
+// With cfg.phi the face potential difference is Phi_R - Phi_L of the given array instead of -g_d h.
 // ---------------------------------------------------------------------------
 void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
     const double lam = dt / cfg.h;
-    fill_ghosts(cfg, G, U);
+    const std::vector<double> PhiP = padded_potential(cfg, G);
+    fill_ghosts(cfg, G, U, PhiP);
 
     Prim W(G.ncell);
     compute_prims(cfg, G, U, W);
@@ -276,14 +322,17 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
         for (c[0] = -G.off[0]; c[0] < G.n[0] + G.off[0]; ++c[0]) {
             if (c[d] + 1 >= G.n[d] + G.off[d]) continue;       // no R cell
             const size_t jL = G.at(c), jR = jL + sd;
+            // S_{i+1/2} = -1/2 (rho_i + rho_{i+1}) (Phi_{i+1} - Phi_i): "gh" = -(Phi_R - Phi_L)
+            const double ghf = PhiP.empty() ? gh : -(PhiP[jR] - PhiP[jL]);
             const Face f = acoustic_face(W.rho[jL], W.u[d][jL], W.p[jL], W.c[jL],
-                                         W.rho[jR], W.u[d][jR], W.p[jR], W.c[jR], gh, cfg.theta);
+                                         W.rho[jR], W.u[d][jR], W.p[jR], W.c[jR], ghf, cfg.theta);
             us[d][jL] = f.ustar; ps[d][jL] = f.pistar; Sf[d][jL] = f.S;
         }
     }
 
     // potential at cell centres (only used by form 1)
     auto Phi = [&](int i, int j, int k) {
+        if (!PhiP.empty()) return PhiP[G.at(i, j, k)];
         return -(cfg.g[0] * (i + 0.5) * cfg.h + cfg.g[1] * (j + 0.5) * cfg.h + cfg.g[2] * (k + 0.5) * cfg.h);
     };
 
@@ -296,7 +345,7 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
         for (c[1] = lo[1]; c[1] < hi[1]; ++c[1])
         for (c[0] = lo[0]; c[0] < hi[0]; ++c[0]) {
             const size_t j = G.at(c);
-            double sum_du = 0.0, sum_dpu = 0.0;
+            double sum_du = 0.0, sum_dpu = 0.0, sum_uS = 0.0;
             double mom[3] = {U.q[1][j], U.q[2][j], U.q[3][j]};
             for (int d = 0; d < cfg.ndim; ++d) {
                 const size_t jm = j - G.stride(d);               // face d- is indexed by its L cell
@@ -304,6 +353,7 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
                 sum_dpu += ps[d][j] * us[d][j] - ps[d][jm] * us[d][jm];           // [Pi* u*]
                 const double Si = 0.5 * (Sf[d][j] + Sf[d][jm]);                   // S_i
                 mom[d] = mom[d] - lam * (ps[d][j] - ps[d][jm]) + lam * Si;
+                sum_uS += 0.5 * (us[d][j] * Sf[d][j] + us[d][jm] * Sf[d][jm]);    // (uS)_i, PAPER.md:544 (App. B)
             }
             const double Lt = 1.0 + lam * sum_du;                                 // L~
             double En = U.q[4][j];
@@ -312,6 +362,7 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
             Ut.q[1][j] = mom[0] / Lt;
             Ut.q[2][j] = mom[1] / Lt;
             Ut.q[3][j] = mom[2] / Lt;
+            if (form == 2) En += lam * sum_uS;                                    // App. B, reading A24
             Ut.q[4][j] = (En - lam * sum_dpu) / Lt;                               // reading A3: divided by L~
         }
     }
@@ -341,6 +392,15 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
                     F[4] += pistar * ustar;                                       // (E~ + Pi*) u*
                     if (form == 1) {
                         // eq. (11) is used as printed: nothing else to add
+                    } else if (form == 2) {
+                        // App. B: the energy source is lam (uS)_i, added once per axis below
+                    } else if (!PhiP.empty()) {
+                        // the same gravity work with a general potential: -lam ( m_+ (Phi_up+ - Phi_i) - m_- (Phi_up- - Phi_i) ),
+                        // Phi_up = Phi of the upwind cell: only inflow faces contribute, with -(Phi_R - Phi_L) of that face
+                        const double m = Ut.q[0][jup] * ustar;
+                        const double ghf = -(PhiP[jR] - PhiP[jL]);
+                        if (side == 1) src[4] += lam * ghf * std::min(m, 0.0);
+                        else           src[4] += lam * ghf * std::max(m, 0.0);
                     } else {
                         // gravity work  -dt {rho u d_x Phi}_i = -lam( [rho~ u* Phi] - [rho~ u*] Phi_i )
                         // with Phi_face = Phi_upwind (reading A13):
@@ -359,6 +419,7 @@ void step(const Cfg& cfg, const Grid& G, State& U, double dt, int form) {
                 }
                 for (int f = 0; f < 5; ++f) dF[f] += Fs[1][f] - Fs[0][f];
                 src[1 + d] += lam * (0.5 * (Sf[d][j] + Sf[d][j - sd]));           // + lam * S_i
+                if (form == 2) src[4] += lam * (0.5 * (us[d][j] * Sf[d][j] + us[d][j - sd] * Sf[d][j - sd]));   // + lam (uS)_i
             }
             double old[5];
             for (int f = 0; f < 5; ++f) old[f] = U.q[f][j];
@@ -412,8 +473,9 @@ void store_dense(const Grid& G, const State& U, double* const out[5]) {
 }
 
 Cfg make_cfg(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa,
-             int theta, const int* bc_type, const double* bc_val) {
+             int theta, const int* bc_type, const double* bc_val, const double* phi = nullptr) {
     Cfg c;
+    c.phi = phi;
     c.n[0] = nx; c.n[1] = ny; c.n[2] = nz;
     c.ndim = nz == 1 ? 2 : 3;
     c.h = h; c.gamma = gamma; c.mu = mu; c.kappa = kappa; c.theta = theta;
@@ -438,11 +500,25 @@ double oracle_K(void) { return K_IMP; }
 // Advance nsteps.  If dts != NULL it holds nsteps prescribed time steps; otherwise each
 // dt = cfl / max_rate (and, if dts_out != NULL, is recorded there).  form: 0 = E + source
 // (normative), 1 = eq. (11).  Returns 0, or -4 if a non-finite rate was met.
+// (2 = Appendix B).  phi: optional dense potential at the cell centres (NULL: constant g).
+int oracle_run_phi(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa,
+                   int theta, const int* bc_type, const double* bc_val,
+                   double* rho, double* rhou, double* rhov, double* rhow, double* E,
+                   int nsteps, double cfl, const double* dts, double* dts_out, int form, const double* phi);
+
 int oracle_run(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa,
                int theta, const int* bc_type, const double* bc_val,
                double* rho, double* rhou, double* rhov, double* rhow, double* E,
                int nsteps, double cfl, const double* dts, double* dts_out, int form) {
-    const Cfg cfg = make_cfg(nx, ny, nz, h, gamma, g, mu, kappa, theta, bc_type, bc_val);
+    return oracle_run_phi(nx, ny, nz, h, gamma, g, mu, kappa, theta, bc_type, bc_val, rho, rhou, rhov, rhow, E, nsteps, cfl, dts,
+                          dts_out, form, nullptr);
+}
+
+int oracle_run_phi(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa,
+                   int theta, const int* bc_type, const double* bc_val,
+                   double* rho, double* rhou, double* rhov, double* rhow, double* E,
+                   int nsteps, double cfl, const double* dts, double* dts_out, int form, const double* phi) {
+    const Cfg cfg = make_cfg(nx, ny, nz, h, gamma, g, mu, kappa, theta, bc_type, bc_val, phi);
     const Grid G(cfg);
     State U(G.ncell);
     const double* in[5] = {rho, rhou, rhov, rhow, E};
@@ -485,7 +561,7 @@ int oracle_fill_ghosts(int nx, int ny, int nz, double h, double gamma, const dou
     State U(G.ncell);
     const double* in[5] = {rho, rhou, rhov, rhow, E};
     load_dense(G, U, in);
-    fill_ghosts(cfg, G, U);
+    fill_ghosts(cfg, G, U, padded_potential(cfg, G));
     double* out[5] = {prho, prhou, prhov, prhow, pE};
     for (int f = 0; f < 5; ++f) if (out[f]) std::memcpy(out[f], U.q[f].data(), G.ncell * sizeof(double));
     return 0;

@@ -25,6 +25,8 @@ def lib():
                   C.c_int, _ip, _dp]
         _lib.oracle_run.argtypes = common + [_dp] * 5 + [C.c_int, C.c_double, _dp, _dp, C.c_int]
         _lib.oracle_run.restype = C.c_int
+        _lib.oracle_run_phi.argtypes = common + [_dp] * 5 + [C.c_int, C.c_double, _dp, _dp, C.c_int, _dp]
+        _lib.oracle_run_phi.restype = C.c_int
         _lib.oracle_max_rate.argtypes = common + [_dp] * 5
         _lib.oracle_max_rate.restype = C.c_double
         _lib.oracle_fill_ghosts.argtypes = common + [_dp] * 10
@@ -66,14 +68,21 @@ def _state(p, U):
 
 def run(p, U, nsteps, cfl=None, dts=None, form=0):
     """Advance a copy of U = [rho, rhou, rhov, rhow, E] (dense, any shape of nx*ny*nz elements,
-    x fastest) by nsteps.  Either dts (array of nsteps prescribed steps) or cfl.  Returns
-    (U_new list of flat arrays, dts_used)."""
+    x fastest) by nsteps.  Either dts (array of nsteps prescribed steps) or cfl.  form: 0 = E + gravity source
+    (normative), 1 = eq. (11), 2 = Appendix B (non-conservative energy); p.get("energy_form") == 1 also selects
+    Appendix B.  p.get("phi"): optional dense potential at the cell centres, else Phi = -g.x.
+    Returns (U_new list of flat arrays, dts_used)."""
     args, keep = _common(p)
     S = _state(p, U)
     dts_in = None if dts is None else np.ascontiguousarray(dts, dtype=np.float64)
     dts_out = np.zeros(max(nsteps, 1))
-    rc = lib().oracle_run(*args, *[_ptr(a) for a in S], int(nsteps),
-                          float(cfl if cfl is not None else 0.0), _ptr(dts_in), _ptr(dts_out), int(form))
+    if form == 0 and int(p.get("energy_form", 0)) == 1:
+        form = 2
+    phi = p.get("phi")
+    phi = None if phi is None else np.ascontiguousarray(np.asarray(phi, dtype=np.float64).reshape(-1))
+    assert phi is None or phi.size == S[0].size
+    rc = lib().oracle_run_phi(*args, *[_ptr(a) for a in S], int(nsteps),
+                              float(cfl if cfl is not None else 0.0), _ptr(dts_in), _ptr(dts_out), int(form), _ptr(phi))
     if rc != 0:
         raise FloatingPointError("oracle: non-finite CFL rate (rc=%d)" % rc)
     return S, dts_out[:nsteps]

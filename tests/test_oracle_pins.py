@@ -727,3 +727,141 @@ def test_strongly_stratified_polytrope_with_flux_bottom_is_steady():
     assert np.abs(S[2] / S[0]).max() < 1e-12
     E0 = U[4].sum()
     assert abs(S[4].sum() - E0) < 1e-12 * E0              # heat in at the bottom = heat out at the top
+
+
+# ----------------------------------------------------------------------------------- Appendix B, general potential
+def _appendix_b_lagrangian_1d(rho, u, v, E, Phi, gamma, lam, K, nsteps):
+    """The non-conservative scheme of Appendix B in the paper's OTHER formulation: the Lagrangian
+    acoustic system in (tau, u, v, E) with its sources -(1/tau) d_m Phi and -(u/tau) d_m Phi, dm = rho dx, face source
+    S_{i+1/2} = -1/2 (1/tau_i + 1/tau_{i+1}) (Phi_{i+1} - Phi_i), then the non-conservative transport
+    form b^{n+1} = b~ - lam [b~ u*] + b~ lam [u*].  Periodic, theta = 1.  Independent of the oracle's flux form."""
+    for _ in range(nsteps):
+        e = E - 0.5 * (u * u + v * v)
+        p = (gamma - 1.0) * rho * e
+        c = np.sqrt(gamma * p / rho)
+        up = lambda f: np.roll(f, -1)
+        a = K * np.maximum(rho * c, up(rho) * up(c))
+        S = -0.5 * (rho + up(rho)) * (up(Phi) - Phi)                                 # face i+1/2
+        us = 0.5 * (u + up(u)) - (up(p) - p - S) / (2 * a)
+        ps = 0.5 * (p + up(p)) - 0.5 * a * (up(u) - u)
+        br = lambda f: f - np.roll(f, 1)                                            # [q]_i
+        Si = 0.5 * (S + np.roll(S, 1))
+        uSi = 0.5 * (us * S + np.roll(us * S, 1))
+        tau_t = 1.0 / rho + lam / rho * br(us)
+        u_t = u - lam / rho * br(ps) + lam / rho * Si
+        E_t = E - lam / rho * br(ps * us) + lam / rho * uSi
+        rho_t = 1.0 / tau_t
+        new = []
+        for b in (rho_t, rho_t * u_t, rho_t * v, rho_t * E_t):
+            bf = np.where(us >= 0, b, up(b))
+            new.append(b - lam * br(bf * us) + b * lam * br(us))
+        rho = new[0]
+        u, v, E = new[1] / rho, new[2] / rho, new[3] / rho
+    return rho, rho * u, rho * v, rho * E
+
+
+def _wave_1d(nx, ny):
+    x = (np.arange(nx) + 0.5) / nx
+    rho = 1.0 + 0.3 * np.sin(2 * np.pi * x)
+    u = 0.4 * np.cos(2 * np.pi * x) - 0.1
+    v = 0.2 * np.sin(4 * np.pi * x)
+    p = 1.0 + 0.2 * np.cos(4 * np.pi * x)
+    E = p / 0.4 / rho + 0.5 * (u * u + v * v)
+    bc = lambda a: np.ascontiguousarray(np.broadcast_to(a[None, None, :], (1, ny, nx)))
+    return x, (rho, u, v, E), [bc(rho), bc(rho * u), bc(rho * v), None, bc(rho * E)], bc
+
+
+def test_appendix_B_scheme_matches_its_lagrangian_formulation_with_a_general_potential():
+    """Oracle form 2 (App. B, reading A24) with an array-valued periodic potential
+    against an independent implementation of the Lagrangian formulation the appendix starts from."""
+    nx, ny = 64, 4
+    x, (rho, u, v, E), U, bc = _wave_1d(nx, ny)
+    Phi = 0.3 * np.sin(2 * np.pi * x) + 0.1 * np.cos(6 * np.pi * x)
+    prm = dict(I.make_params(nx, ny, 1, 1.0 / nx, 1.4, theta=0), phi=bc(Phi))
+    dt = 0.2 * (1.0 / nx) / 2.0
+    n = 25
+    S, _ = O.run(prm, U, n, dts=np.full(n, dt), form=2)
+    ref = _appendix_b_lagrangian_1d(rho, u, v, E, Phi, 1.4, dt * nx, O.K(), n)
+    for f, r in zip((0, 1, 2, 4), ref):
+        assert np.abs(S[f].reshape(ny, nx) - r[None, :]).max() < 1e-13, f
+    # the potential really acted, and the energy form matters: form 0 gives another energy, the same mass
+    S0, _ = O.run(dict(prm, phi=None), U, n, dts=np.full(n, dt), form=2)
+    assert np.abs(S0[1] - S[1]).max() > 1e-3
+    Sc, _ = O.run(prm, U, n, dts=np.full(n, dt), form=0)
+    assert np.abs(Sc[4] - S[4]).max() > 1e-7 and np.abs(Sc[4] - S[4]).max() < 1e-2
+
+
+def test_appendix_B_coincides_with_the_conservative_scheme_where_it_must():
+    """Without gravity the two energy updates are the same expression (S = 0): bit-identical.  At rest in a
+    hydrostatic column u* = 0 on every face, so (uS)_i = 0 and the well-balanced property carries
+    over: the isothermal atmosphere stays at rest.  With gravity and flow the total energy sum(E + rho Phi) is conserved
+    to round-off by the conservative forms only."""
+    prm, U = I.random_state(18, 14, 6, 41, mu=1e-3, kappa=2e-3)
+    A, _ = O.run(prm, U, 4, cfl=0.4, form=0)
+    B, _ = O.run(prm, U, 4, cfl=0.4, form=2)
+    for f in range(5):
+        assert np.array_equal(A[f], B[f]), f
+    prm, U = I.config1_atmosphere(32, amp=0.0)
+    S, _ = O.run(prm, U, 300, cfl=0.4, form=2)
+    assert np.abs(S[2] / S[0]).max() < 1e-13
+    prm, U = I.config1_atmosphere(32, amp=1e-2)
+    y = (np.arange(32) + 0.5) / 32
+    tot = lambda S: (S[4].reshape(32, 32) + S[0].reshape(32, 32) * y[:, None]).sum()
+    e0 = (U[4][0] + U[0][0] * y[:, None]).sum()
+    A, _ = O.run(prm, U, 50, cfl=0.4, form=0)
+    B, _ = O.run(prm, U, 50, cfl=0.4, form=2)
+    assert abs(tot(A) - e0) < 1e-12 * e0
+    assert 1e-12 * e0 < abs(tot(B) - e0) < 1e-5 * e0
+    assert abs(B[0].sum() - U[0].sum()) < 1e-13 * U[0].sum()
+
+
+def test_array_potential_reduces_to_constant_gravity_and_keeps_the_two_energy_forms_equivalent():
+    """S_{i+1/2} = -1/2 (rho_i + rho_{i+1}) (Phi_{i+1} - Phi_i).  (a) Phi = -g.x sampled at the cell
+    centres (values exactly representable: h = 1/16, g = (0.5, -1, 0.25)) reproduces the constant-g run: the face sources
+    are bit-identical, the gravity work differs only by the rounding of lam (g h) m against dt g m.  (b) With a smooth
+    non-linear potential the rho E + source form and the calligraphic-E form (11) still agree to round-off,
+    which pins the upwind-potential gravity work.  (c) A column in discrete hydrostatic balance (14) with that potential
+    stays at rest."""
+    PERp, REFp = I.BC_PERIODIC, I.BC_REFLECTING
+    n = 16
+    h = 1.0 / n
+    g = (0.5, -1.0, 0.25)
+    prm, U = I.random_state(n, n, n, 43, g=g, h=h, mu=1e-3, kappa=1e-3,
+                            bc_type=((REFp, REFp), (REFp, I.BC_FIXED_T), (REFp, REFp)), bc_value=((0, 0), (0, 2.5), (0, 0)))
+    c = (np.arange(n) + 0.5) * h
+    Phi = -(g[0] * c[None, None, :] + g[1] * c[None, :, None] + g[2] * c[:, None, None])
+    A, dts = O.run(prm, U, 5, cfl=0.4)
+    B, _ = O.run(dict(prm, phi=Phi), U, 5, dts=dts)
+    for f in range(4):
+        assert np.array_equal(A[f], B[f]) or np.abs(A[f] - B[f]).max() < 2e-15 * np.abs(A[f]).max(), f
+    assert np.abs(A[4] - B[4]).max() < 1e-14 * np.abs(A[4]).max()
+    # (b) non-linear potential, periodic in x and y, walls in z
+    prm, U = I.random_state(12, 10, 8, 44, bc_type=((PERp, PERp), (PERp, PERp), (REFp, REFp)), h=1.0 / 12)
+    x = (np.arange(12) + 0.5) / 12
+    yy = (np.arange(10) + 0.5) / 10
+    z = (np.arange(8) + 0.5) / 12
+    Phi = 0.2 * np.sin(2 * np.pi * x)[None, None, :] * np.cos(2 * np.pi * yy)[None, :, None] + (0.8 * z + 0.5 * z * z)[:, None, None]
+    pp = dict(prm, phi=Phi)
+    A, dts = O.run(pp, U, 6, cfl=0.3, form=0)
+    B, _ = O.run(pp, U, 6, dts=dts, form=1)
+    for f in range(5):
+        assert np.abs(A[f] - B[f]).max() < 5e-14 * np.abs(A[f]).max(), f
+    etot = lambda S: (S[4] + S[0] * Phi.reshape(-1)).sum()
+    e0 = (U[4] + U[0] * Phi).sum()
+    assert abs(etot(A) - e0) < 1e-13 * abs(e0)                 # sum (E + rho Phi) is conserved (PAPER.md:61-64)
+    assert np.abs(A[3] - O.run(prm, U, 6, dts=dts)[0][3]).max() > 1e-3   # and the potential really acted
+    # (c) hydrostatic column in a non-uniform field g(y) = 1 + y: Phi = y + y^2 / 2, T = 1, recursion (14) with the local dPhi
+    ny = 48
+    hy = 1.0 / ny
+    yc = (np.arange(ny) + 0.5) * hy
+    Phic = yc + 0.5 * yc * yc
+    rho = np.empty(ny)
+    rho[0] = 1.0
+    for j in range(ny - 1):
+        d = Phic[j + 1] - Phic[j]
+        rho[j + 1] = rho[j] * (1.0 - 0.5 * d) / (1.0 + 0.5 * d)
+    prmc = I.make_params(8, ny, 1, hy, 1.4, bc_type=((PERp, PERp), (REFp, REFp), (0, 0)))
+    col = lambda a: np.ascontiguousarray(np.broadcast_to(a[None, :, None], (1, ny, 8)))
+    Uc = [col(rho), col(0 * rho), col(0 * rho), None, col(rho / 0.4)]
+    S, _ = O.run(dict(prmc, phi=col(Phic)), Uc, 400, cfl=0.4)
+    assert np.abs(S[2] / S[0]).max() < 1e-13
