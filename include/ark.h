@@ -22,7 +22,8 @@
  *     attributes live there): calling an entry point while another device is current returns ARK_EINVAL.
  *   - Every entry point returns an ARK_* code and never throws; ark_last_error() gives a text for
  *     the last failure on the calling thread.
- *   - Gravity is the constant vector g (Phi = -g.x, never stored: A12).  The acoustic impedance
+ *   - Gravity is the constant vector g (Phi = -g.x, never stored: A12) unless ark_set_potential supplies an array.
+ *     The acoustic impedance
  *     constant is K = 1.1 (a = K max(rho_L c_L, rho_R c_R), A2), reported by
  *     ark_version_string().
  */
@@ -94,6 +95,27 @@ int ark_step(ark_solver*, double dt);
  * After the first step, pairs of steps are replayed from a CUDA graph captured on a stream of the library's own
  * (ordered with the caller's stream through events): the small 2D configurations are launch-latency-bound. */
 int ark_run(ark_solver*, int nsteps, double cfl, double* dts_out);
+
+/* Energy update (PAPER.md:194-210 and Appendix B, :514-546).  ARK_ENERGY_CONSERVATIVE (default): rho*E advanced in
+ * flux form with the mass-flux-weighted gravity work, which conserves sum (E + rho Phi) to
+ * round-off.  ARK_ENERGY_APPENDIX_B: the non-conservative scheme of Appendix B; mass and momentum are unchanged, the
+ * energy carries the source (dt/dx) (uS)_i, (uS)_i = 1/2 (u*_{i+1/2} S_{i+1/2} + u*_{i-1/2} S_{i-1/2}) summed over the
+ * axes, in the acoustic and in the final update (reading A24 of DESIGN.md).  Takes effect at the
+ * next step.  Errors: ARK_EINVAL. */
+enum { ARK_ENERGY_CONSERVATIVE = 0, ARK_ENERGY_APPENDIX_B = 1 };
+int ark_set_energy_form(ark_solver*, int form);
+
+/* Array-valued gravitational potential Phi(x) (S_{i+1/2} = -1/2 (rho_i + rho_{i+1}) (Phi_{i+1} - Phi_i),
+ * PAPER.md:152; gravity work with the upwind potential; ghost-cell density from relation (14) with the
+ * potential difference).  d_phi: DEVICE array, dense interior values at the cell centres (nx*ny*nz, x
+ * fastest), copied; ghost values (reading A25): periodic axes wrap, wall axes continue Phi linearly, which reproduces a
+ * constant gravity exactly.  d_buffer: caller-allocated DEVICE memory of at least ark_potential_bytes(nx, ny, nz) bytes,
+ * 256-byte aligned, which the library keeps using (padded potential) until ark_destroy or the next ark_set_potential; the
+ * caller owns it.  While a potential is set, the vector g of ark_create is ignored and ark_diagnostics uses Phi for the
+ * total energy.  d_phi == NULL returns to the constant g (buffer ignored).  Algorithmic traffic of a step rises from 80
+ * to 88 B per cell update in 3D (64 -> 72 B in 2D).  Asynchronous on the stream.  Errors: ARK_EINVAL, ARK_ECUDA. */
+size_t ark_potential_bytes(int nx, int ny, int nz);
+int ark_set_potential(ark_solver*, const double* d_phi, void* d_buffer, size_t buffer_bytes);
 
 /* Diagnostics of the current state as the paper reports them (PAPER.md:398-407 maximum velocity, :435 mean absolute
  * velocity, :14 conserved mass and total energy).  out (HOST, 6 doubles) = { max |u|, mean |u|, kinetic energy

@@ -16,7 +16,8 @@ ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
 BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
-           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_diagnostics", "ark_debug_get_padded",
+           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
+           "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
 
 
@@ -59,6 +60,12 @@ def load():
     lib.ark_diagnostics.restype = ip
     lib.ark_run.argtypes = [vp, ip, C.c_double, C.POINTER(C.c_double)]
     lib.ark_run.restype = ip
+    lib.ark_set_energy_form.argtypes = [vp, ip]
+    lib.ark_set_energy_form.restype = ip
+    lib.ark_potential_bytes.argtypes = [ip, ip, ip]
+    lib.ark_potential_bytes.restype = C.c_size_t
+    lib.ark_set_potential.argtypes = [vp, dp, vp, C.c_size_t]
+    lib.ark_set_potential.restype = ip
     lib.ark_step_kernel_timing.argtypes = [vp, ip]
     lib.ark_step_kernel_timing.restype = ip
     lib.ark_step_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int)]
@@ -100,7 +107,8 @@ class Solver:
 
     params: dict(nx, ny, nz, dx, gamma, g, mu, kappa, theta, bc_type[3][2], bc_value[3][2]) as produced by
     `paper_1903_09043_b200.inputs`.  State tensors are dense float64 CUDA tensors of nx*ny*nz elements
-    (x fastest); rhow is None in 2D.
+    (x fastest); rhow is None in 2D.  Optional keys: energy_form (1 = Appendix B, ark_set_energy_form) and phi (dense
+    potential at the cell centres, ark_set_potential).
     """
 
     def __init__(self, params, device="cuda:0", stream=None):
@@ -132,6 +140,29 @@ class Solver:
                               C.c_void_p(self._ws_ptr), C.c_size_t(nbytes), C.c_void_p(self.stream.cuda_stream)))
         self._h = h
         self._lib = lib
+        self._phi_buf = None
+        if int(params.get("energy_form", 0)) != 0:
+            self.set_energy_form(int(params["energy_form"]))
+        if params.get("phi") is not None:
+            self.set_potential(torch.as_tensor(params["phi"], dtype=torch.float64).reshape(-1).to(self.device))
+
+    # ------------------------------------------------------------------ general path (Appendix B, array-valued potential)
+    def set_energy_form(self, form):
+        _check(self._lib.ark_set_energy_form(self._h, int(form)))
+
+    def set_potential(self, phi):
+        """phi: dense float64 CUDA tensor of nx*ny*nz elements (potential at the cell centres), or None for constant g."""
+        if phi is None:
+            _check(self._lib.ark_set_potential(self._h, None, None, 0))
+            self._phi_buf = None
+            return
+        if phi.dtype != torch.float64 or not phi.is_contiguous() or phi.numel() != self.n or phi.device.type != "cuda":
+            raise ValueError("phi must be a contiguous float64 CUDA tensor of %d elements" % self.n)
+        nbytes = int(self._lib.ark_potential_bytes(self.nx, self.ny, self.nz))
+        buf = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (buf.data_ptr() + 255) // 256 * 256
+        _check(self._lib.ark_set_potential(self._h, C.c_void_p(phi.data_ptr()), C.c_void_p(ptr), C.c_size_t(nbytes)))
+        self._phi_buf = buf                      # the library keeps using it (caller-owned): keep it alive
 
     # ------------------------------------------------------------------ state
     def _ptrs(self, U, host=False):

@@ -30,7 +30,7 @@ constexpr int TX3 = ARK_TX3, NW3 = ARK_NW3;   // 3D: outputs per row, row pairs 
 constexpr int TY3 = 2 * NW3 - 4;
 constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
 
-#define ARK_KERNEL_REV "r2.1"
+#define ARK_KERNEL_REV "r2.2"
 constexpr int CFL_BLOCK = 256;
 #define ARK_MAX_TIMED 4096
 constexpr int MAX_SCRATCH = 1 << 16;          // per-block rate slots
@@ -149,14 +149,13 @@ int grid_for(long long n, int block, int cap = 148 * 8) {
     return (int)(b < cap ? b : cap);
 }
 
-template <int NDIM, bool VISC, int TX, int TY>
-int launch_step_t(ark_solver* s, double dt, const double* dt_dev) {
-    using C = ArkStepCfg<NDIM, VISC, TX, TY>;
-    auto kern = ark_k_step<NDIM, VISC, TX, TY>;
+template <bool VISC, bool GEN>
+int launch_step2(ark_solver* s, double dt, const double* dt_dev) {
+    using C = ArkStepCfg<2, VISC, TX2, TY2>;
+    auto kern = ark_k_step<2, VISC, GEN, TX2, TY2>;
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
     if (timed) ARK_CUDA(cudaEventRecord(s->timer->ev0[s->n_timed], s->stream));
-    kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
-                                                            s->scratch, s->zchunk, s->tmap[s->cur]);
+    kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev, s->scratch);
     if (timed) { ARK_CUDA(cudaEventRecord(s->timer->ev1[s->n_timed], s->stream)); s->n_timed++; }
     ARK_CUDA(cudaGetLastError());
     s->launches++;
@@ -192,10 +191,10 @@ int launch_bc(ark_solver* s, double* U) {
     return ARK_OK;
 }
 
-template <bool VISC, bool GXY>
+template <bool VISC, bool GXY, bool GEN>
 int launch_step3(ark_solver* s, double dt, const double* dt_dev) {
     using C = ArkCfg3<VISC, TX3, NW3>;
-    auto kern = ark_k_step3<VISC, GXY, TX3, NW3>;
+    auto kern = ark_k_step3<VISC, GXY, GEN, TX3, NW3>;
     const bool timed = s->timing && s->n_timed < ARK_MAX_TIMED;
     if (timed) ARK_CUDA(cudaEventRecord(s->timer->ev0[s->n_timed], s->stream));
     kern<<<s->step_grid, C::NT, C::SMEM_BYTES, s->stream>>>(s->P, s->U[s->cur], s->U[1 - s->cur], dt, dt_dev,
@@ -207,29 +206,44 @@ int launch_step3(ark_solver* s, double dt, const double* dt_dev) {
 }
 
 // opt-in to the large dynamic shared memory of the step kernels on the CURRENT device (the attribute is per device)
-int set_step_attributes(int ndim) {
-    if (ndim == 3) {
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<true, true, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<true, TX3, NW3>::SMEM_BYTES));
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<true, false, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<true, TX3, NW3>::SMEM_BYTES));
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<false, true, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<false, TX3, NW3>::SMEM_BYTES));
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step3<false, false, TX3, NW3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkCfg3<false, TX3, NW3>::SMEM_BYTES));
-    } else {
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step<2, true, TX2, TY2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkStepCfg<2, true, TX2, TY2>::SMEM_BYTES));
-        ARK_CUDA(cudaFuncSetAttribute(ark_k_step<2, false, TX2, TY2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ArkStepCfg<2, false, TX2, TY2>::SMEM_BYTES));
-    }
+template <typename K>
+int set_smem(K kern, size_t bytes) {
+    ARK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     return ARK_OK;
+}
+int set_step_attributes(int ndim) {
+    int rc = ARK_OK;
+    if (ndim == 3) {
+        const size_t bv = ArkCfg3<true, TX3, NW3>::SMEM_BYTES, bi = ArkCfg3<false, TX3, NW3>::SMEM_BYTES;
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<true, true, false, TX3, NW3>, bv);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<true, false, false, TX3, NW3>, bv);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<true, true, true, TX3, NW3>, bv);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<false, true, false, TX3, NW3>, bi);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<false, false, false, TX3, NW3>, bi);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step3<false, true, true, TX3, NW3>, bi);
+    } else {
+        const size_t bv = ArkStepCfg<2, true, TX2, TY2>::SMEM_BYTES, bi = ArkStepCfg<2, false, TX2, TY2>::SMEM_BYTES;
+        if (rc == ARK_OK) rc = set_smem(ark_k_step<2, true, false, TX2, TY2>, bv);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step<2, true, true, TX2, TY2>, bv);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step<2, false, false, TX2, TY2>, bi);
+        if (rc == ARK_OK) rc = set_smem(ark_k_step<2, false, true, TX2, TY2>, bi);
+    }
+    return rc;
 }
 
 int do_step(ark_solver* s, double dt, const double* dt_dev) {
     int rc = launch_bc(s, s->U[s->cur]);
     if (rc != ARK_OK) return rc;
     const bool visc = s->P.mu > 0.0 || s->P.kappa > 0.0;
+    const bool gen = s->P.phi != nullptr || s->P.eform != 0;    // general path: array-valued potential and / or Appendix B
     if (s->P.ndim == 3) {
         const bool gxy = s->P.D.g_on[0] || s->P.D.g_on[1];
-        if (visc) rc = gxy ? launch_step3<true, true>(s, dt, dt_dev) : launch_step3<true, false>(s, dt, dt_dev);
-        else      rc = gxy ? launch_step3<false, true>(s, dt, dt_dev) : launch_step3<false, false>(s, dt, dt_dev);
+        if (gen)       rc = visc ? launch_step3<true, true, true>(s, dt, dt_dev) : launch_step3<false, true, true>(s, dt, dt_dev);
+        else if (visc) rc = gxy ? launch_step3<true, true, false>(s, dt, dt_dev) : launch_step3<true, false, false>(s, dt, dt_dev);
+        else           rc = gxy ? launch_step3<false, true, false>(s, dt, dt_dev) : launch_step3<false, false, false>(s, dt, dt_dev);
     } else {
-        rc = visc ? launch_step_t<2, true, TX2, TY2>(s, dt, dt_dev) : launch_step_t<2, false, TX2, TY2>(s, dt, dt_dev);
+        if (gen) rc = visc ? launch_step2<true, true>(s, dt, dt_dev) : launch_step2<false, true>(s, dt, dt_dev);
+        else     rc = visc ? launch_step2<true, false>(s, dt, dt_dev) : launch_step2<false, false>(s, dt, dt_dev);
     }
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
@@ -617,6 +631,48 @@ int ark_diagnostics(ark_solver* s, double* out) {
     out[3] = h[3];                 // max Mach number
     out[4] = h[4] * vol;           // mass
     out[5] = h[5] * vol;           // total energy incl. potential
+    return ARK_OK;
+}
+
+int ark_set_energy_form(ark_solver* s, int form) {
+    if (!s || (form != ARK_ENERGY_CONSERVATIVE && form != ARK_ENERGY_APPENDIX_B)) return fail(ARK_EINVAL, "ark_set_energy_form: form must be 0 or 1%s");
+    s->P.eform = form;
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }   // the captured launches carry the old parameters
+    return ARK_OK;
+}
+
+size_t ark_potential_bytes(int nx, int ny, int nz) {
+    if (!supported_grid(nx, ny, nz)) return 0;
+    return (size_t)make_layout(nx, ny, nz).fstride * sizeof(double);
+}
+
+int ark_set_potential(ark_solver* s, const double* d_phi, void* d_buffer, size_t buffer_bytes) {
+    if (!s) return fail(ARK_EINVAL, "ark_set_potential: NULL handle%s");
+    ARK_ON_DEVICE(s);
+    ArkParams& P = s->P;
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    if (!d_phi) {                                   // back to the constant gravity vector of ark_create
+        P.phi = nullptr;
+        ark_fill_derived(P);
+        return ARK_OK;
+    }
+    const size_t need = (size_t)P.fstride * sizeof(double);
+    if (!d_buffer || buffer_bytes < need || ((size_t)d_buffer & 255))
+        return fail(ARK_EINVAL, "ark_set_potential: buffer NULL, misaligned (256 B) or smaller than ark_potential_bytes()%s");
+    double* pad = (double*)d_buffer;
+    ARK_CUDA(cudaMemsetAsync(pad, 0, need, s->stream));
+    const long long n = (long long)P.nx * P.ny * P.nz;
+    ark_k_pack<<<grid_for(n, 256), 256, 0, s->stream>>>(P, pad, d_phi, 0);
+    ark_k_phi_ghosts<0><<<grid_for((long long)P.ny * P.nz, 128), 128, 0, s->stream>>>(P, pad);
+    ark_k_phi_ghosts<1><<<grid_for((long long)(P.nx + 2 * ARK_NG) * P.nz, 128), 128, 0, s->stream>>>(P, pad);
+    s->launches += 3;
+    if (P.ndim == 3) {
+        ark_k_phi_ghosts<2><<<grid_for((long long)(P.nx + 2 * ARK_NG) * (P.ny + 2 * ARK_NG), 128), 128, 0, s->stream>>>(P, pad);
+        s->launches++;
+    }
+    ARK_CUDA(cudaGetLastError());
+    P.phi = pad;
+    for (int d = 0; d < P.ndim; ++d) P.D.g_on[d] = 1;          // every axis carries gravity terms now
     return ARK_OK;
 }
 

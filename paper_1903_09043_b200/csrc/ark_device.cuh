@@ -51,6 +51,11 @@ struct ArkParams {
     int bc[3][2];
     double bcv[3][2];
     ArkDerived D;
+    // general path: energy form (0: rho*E with the gravity work of PAPER.md:204-208;
+    // 1: the non-conservative scheme of Appendix B) and an optional array-valued potential
+    // (PAPER.md:55, :152), padded like a state field with its ghost values already filled (reading A25); NULL = -g.x
+    int eform;
+    const double* phi;
 };
 
 inline void ark_fill_derived(ArkParams& P) {
@@ -156,6 +161,11 @@ ARK_DEV void ark_mbar_wait(unsigned long long* bar, unsigned parity) {
 // used; ark_tm_wait_st() orders earlier stores before later loads of the same columns.
 // ------------------------------------------------------------------------------------------------
 #ifndef ARK_HOST_EMU
+// ARK_TM_CLOBBER: "memory" makes every TMEM transfer a scheduling fence for shared / global accesses (TMEM is not
+// memory the compiler knows about: the volatile asm statements keep their own relative order)
+#ifndef ARK_TM_CLOBBER
+#define ARK_TM_CLOBBER "memory"
+#endif
 #define ARK_LO(x) "r"(__double2loint(x))
 #define ARK_HI(x) "r"(__double2hiint(x))
 ARK_DEV unsigned ark_tm_alloc_all(unsigned* slot_in_smem) {           // one full warp; 512 columns = the whole TMEM
@@ -171,14 +181,14 @@ ARK_DEV void ark_tm_fence_after_sync() { asm volatile("tcgen05.fence::after_thre
 ARK_DEV void ark_tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 ARK_DEV void ark_tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 ARK_DEV void ark_tm_st1(unsigned a, double v0) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(a), ARK_LO(v0), ARK_HI(v0) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(a), ARK_LO(v0), ARK_HI(v0) : ARK_TM_CLOBBER);
 }
 ARK_DEV void ark_tm_st2(unsigned a, double v0, double v1) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1) : ARK_TM_CLOBBER);
 }
 ARK_DEV void ark_tm_ld2(unsigned a, double& v0, double& v1) {
     int l0, h0, l1, h1;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1) : "r"(a) : "memory");
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1);
 }
 // ARK_TM_GRAN: doubles moved per tcgen05 instruction.  Wide transfers need their 2*GRAN registers contiguous, which
@@ -189,7 +199,7 @@ ARK_DEV void ark_tm_ld2(unsigned a, double& v0, double& v1) {
 #if ARK_TM_GRAN >= 4
 ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1),
-                 ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3) : "memory");
+                 ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3) : ARK_TM_CLOBBER);
 }
 #elif ARK_TM_GRAN == 2
 ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) { ark_tm_st2(a, v0, v1); ark_tm_st2(a + 4, v2, v3); }
@@ -200,7 +210,7 @@ ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) 
 ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(a),
                  ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3), ARK_LO(v4), ARK_HI(v4),
-                 ARK_LO(v5), ARK_HI(v5), ARK_LO(v6), ARK_HI(v6), ARK_LO(v7), ARK_HI(v7) : "memory");
+                 ARK_LO(v5), ARK_HI(v5), ARK_LO(v6), ARK_HI(v6), ARK_LO(v7), ARK_HI(v7) : ARK_TM_CLOBBER);
 }
 #else
 ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
@@ -209,14 +219,14 @@ ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, 
 #endif
 ARK_DEV void ark_tm_ld1(unsigned a, double& v0) {
     int l0, h0;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(l0), "=r"(h0) : "r"(a) : "memory");
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(l0), "=r"(h0) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0);
 }
 #if ARK_TM_GRAN >= 4
 ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) {
     int l0, h0, l1, h1, l2, h2, l3, h3;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3) : "r"(a) : "memory");
+                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
 }
 #elif ARK_TM_GRAN == 2
@@ -229,7 +239,7 @@ ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& 
     int l0, h0, l1, h1, l2, h2, l3, h3, l4, h4, l5, h5, l6, h6, l7, h7;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
                  : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3), "=r"(l4), "=r"(h4), "=r"(l5), "=r"(h5),
-                   "=r"(l6), "=r"(h6), "=r"(l7), "=r"(h7) : "r"(a) : "memory");
+                   "=r"(l6), "=r"(h6), "=r"(l7), "=r"(h7) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
     v4 = __hiloint2double(h4, l4); v5 = __hiloint2double(h5, l5); v6 = __hiloint2double(h6, l6); v7 = __hiloint2double(h7, l7);
 }
@@ -352,7 +362,8 @@ ARK_GLOBAL void ark_k_unpack_padded(ArkParams P, const double* __restrict__ U, d
 //   fixed-T no-slip wall: u -> -u (all components), T_g = 2 T_w - T_src.
 //   imposed-flux wall (A22): u_n -> -u_n, T_g = T_src + (2l-1) F h / kappa (F = heat flux entering).
 //   rho_g from the discrete hydrostatic relation (14), PAPER.md:237:
-//       p_g - p_prev = 1/2 (rho_prev + rho_g) delta,  delta = Phi_prev - Phi_g = -+ g_d h,  p_g = rho_g T_g.
+//       p_g - p_prev = 1/2 (rho_prev + rho_g) delta,  delta = Phi_prev - Phi_g = -+ g_d h,  p_g = rho_g T_g
+//       (with an array-valued potential, P.phi: the difference of its padded values).
 // ------------------------------------------------------------------------------------------------
 template <int AXIS>
 ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
@@ -404,7 +415,7 @@ ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
                 ug[0] = -ug[0]; ug[1] = -ug[1]; ug[2] = -ug[2];
                 Tg = 2.0 * P.bcv[AXIS][side] - ws.T;
             }
-            const double delta = (side == 0 ? -1.0 : 1.0) * P.g[AXIS] * P.h;
+            const double delta = P.phi ? P.phi[jp] - P.phi[jg] : (side == 0 ? -1.0 : 1.0) * P.g[AXIS] * P.h;
             double rg = (wp.p + 0.5 * wp.rho * delta) / (Tg - 0.5 * delta);
             // A9 needs T_g > |g_d| h / 2: otherwise relation (14) has no positive solution; flag the cell (NaN reaches the
             // CFL reduction, which reports ARK_ENONFINITE) instead of marching on with a negative ghost density
@@ -444,6 +455,35 @@ ARK_GLOBAL void ark_k_bc_x_periodic(ArkParams P, double* __restrict__ U) {
         const double a = U[src], b = U[src + 1];
         U[dst] = a; U[dst + 1] = b;
         (void)vec;
+    }
+}
+
+// Ghost values of an array-valued potential (reading A25): periodic axes wrap, wall axes continue Phi
+// linearly from the two cells next to the wall (Phi(-l) = Phi(0) + l (Phi(0) - Phi(1))), which reproduces a constant
+// gravity exactly.  Same x, y, z sweep order over the already-extended ranges as the state's ghost fill; runs once, in
+// ark_set_potential.  One thread per (transverse position).
+template <int AXIS>
+ARK_GLOBAL void ark_k_phi_ghosts(ArkParams P, double* __restrict__ phi) {
+    int na, nb, loa, lob;
+    if (AXIS == 0)      { na = P.ny;            loa = 0;        nb = P.nz;                        lob = 0; }
+    else if (AXIS == 1) { na = P.nx + 2 * ARK_NG; loa = -ARK_NG; nb = P.nz;                        lob = 0; }
+    else                { na = P.nx + 2 * ARK_NG; loa = -ARK_NG; nb = P.ny + 2 * ARK_NG;           lob = -ARK_NG; }
+    const long long ntr = (long long)na * nb;
+    const int n = AXIS == 0 ? P.nx : (AXIS == 1 ? P.ny : P.nz);
+    const long long sd = AXIS == 0 ? 1 : (AXIS == 1 ? (long long)P.px : (long long)P.px * P.py);
+    for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < ntr; r += (long long)gridDim.x * blockDim.x) {
+        const int a = loa + (int)(r % na), b = lob + (int)(r / na);
+        const long long base = AXIS == 0 ? ark_idx(P, 0, a, b) : (AXIS == 1 ? ark_idx(P, a, 0, b) : ark_idx(P, a, b, 0));
+        for (int l = 1; l <= ARK_NG; ++l) {
+            if (P.bc[AXIS][0] == ARK_BCK_PERIODIC) {
+                phi[base - l * sd] = phi[base + (n - l) * sd];
+                phi[base + (n - 1 + l) * sd] = phi[base + (l - 1) * sd];
+            } else {
+                const double p0 = phi[base], p1 = phi[base + sd], q0 = phi[base + (n - 1) * sd], q1 = phi[base + (n - 2) * sd];
+                phi[base - l * sd] = p0 + l * (p0 - p1);
+                phi[base + (n - 1 + l) * sd] = q0 + l * (q0 - q1);
+            }
+        }
     }
 }
 
@@ -544,7 +584,7 @@ ARK_GLOBAL void ark_k_diag_pass1(ArkParams P, const double* __restrict__ U, doub
         const double ke = 0.5 * m2 * rinv;
         const double speed = sqrt(m2) * rinv;
         const double cs = sqrt(P.gamma * P.gm1 * (E - ke) * rinv);
-        const double phi = -((i + 0.5) * P.g[0] + (j + 0.5) * P.g[1] + (P.ndim == 3 ? (k + 0.5) * P.g[2] : 0.0)) * P.h;
+        const double phi = P.phi ? P.phi[c] : -((i + 0.5) * P.g[0] + (j + 0.5) * P.g[1] + (P.ndim == 3 ? (k + 0.5) * P.g[2] : 0.0)) * P.h;
         const double w[ARK_NDIAG] = {speed, speed, ke, speed / cs, rho, E + rho * phi};
         ark_diag_combine(v, w);
     }

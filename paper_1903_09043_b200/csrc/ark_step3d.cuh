@@ -102,6 +102,12 @@ struct ArkMarch3 {
     unsigned tm;                         // TMEM address of this thread's scratch columns
     int tcur;                            // TMEM primitive slot of plane q (the other one holds q-1, then q+1)
     ark_u64 rate_max;
+    // general path only (GEN; see ark_step.cuh): array-valued potential, read straight from global memory
+    const double* php;                   // plane q+1 of the padded potential at this lane's column (row 0 of the array)
+    int pho[4];                          // row offsets (doubles) of rows a-1, a, b, b+1, clamped to the padded array
+    double phc[2];                       // Phi(q) of the own two columns
+    double ghz[2];                       // -(Phi(q) - Phi(q-1)) of the own two columns: the z face (q-1|q)
+    double ghyu_prev;                    // -(Phi_{b+1} - Phi_b) at plane q-1: the high-y face of row b, used one plane later
 };
 
 template <bool VISC, int TX, int NW>
@@ -315,8 +321,9 @@ ARK_DEV void ark_face_flux_n(double (*F)[5], const bool* left, const double* con
 }
 
 // GXY: gravity may have x / y components (false: only g_z, the x and y source terms vanish at compile time)
-template <bool VISC, bool GXY, int TX, int NW, int ROLE, bool STEADY>
+template <bool VISC, bool GXY, bool GEN, int TX, int NW, int ROLE, bool STEADY>
 ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VISC, TX, NW>& M, const int q) {
+    static_assert(!GEN || GXY, "the general path keeps all gravity components");
     using C = ArkCfg3<VISC, TX, NW>;
     constexpr int RX = C::RX, NCOL = C::NCOL, NP = C::NP, NT = C::NS;   // NT: stride of the exchange arrays
     constexpr int R0 = ROLE == 0 ? 1 : 0, R1 = ROLE == 2 ? 0 : 1, NA = R1 - R0 + 1;   // active (ring / tile) rows of the pair
@@ -329,6 +336,27 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     const double ghx = GXY ? P.D.gh[0] : 0.0, ghy = GXY ? P.D.gh[1] : 0.0;
     const unsigned tm = M.tm;
     const int tcur = M.tcur;
+    // GEN: every face has its own -(Phi_R - Phi_L) in place of g_d h; the gravity work
+    // is lam * that difference * the inflowing mass flux, or, for Appendix B (P.eform == 1), replaced by lam (uS)_i
+    const bool PH = GEN && P.phi != nullptr;
+    const bool eformB = GEN && P.eform == 1;
+    const bool wk = !eformB;
+    double ghxl[2] = {ghx, ghx}, ghxh[2] = {ghx, ghx}, ghzh[2] = {P.D.gh[2], P.D.gh[2]}, ghyi = ghy, ghyl = ghy, ghyu = ghy;
+    if (PH) {
+        const double* pq1 = M.php;                        // plane q+1
+        const double* pq0 = M.php - M.pstride;            // plane q
+        ghyi = M.phc[0] - M.phc[1];
+        if (ROLE != 0) ghyl = pq0[M.pho[0]] - M.phc[0];
+        if (ROLE != 2) ghyu = M.phc[1] - pq0[M.pho[3]];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const double phn = pq1[M.pho[1 + r]];
+            ghzh[r] = M.phc[r] - phn;
+            ghxl[r] = ark_xl(M.phc[r]) - M.phc[r];
+            ghxh[r] = ark_xr(ghxl[r]);
+            M.phc[r] = phn;                               // (the differences of plane q are complete: rotate)
+        }
+    }
 
     // ---------------- S1: primitives of plane q (parked in TMEM one iteration ago) and, for the viscous z stencil,
     // u,v,w,T of plane q-1; prefetch plane q+2; primitives of plane q+1 of the own two columns
@@ -388,13 +416,13 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
 #pragma unroll
         for (int r = R0; r <= R1; ++r) {
             const ArkPrim& c = wc[r];
-            in[r - R0] = ark_face_in(ghx, lr[r], Lu[r], lp[r], lrc[r], lirc[r], c.rho, c.u, c.p, c.rc, c.irc);
-            in[NA + r - R0] = ark_face_in(P.D.gh[2], c.rho, c.w, c.p, c.rc, c.irc, wn[r].rho, wn[r].w, wn[r].p, wn[r].rc, wn[r].irc);
+            in[r - R0] = ark_face_in(GEN ? ghxl[r] : ghx, lr[r], Lu[r], lp[r], lrc[r], lirc[r], c.rho, c.u, c.p, c.rc, c.irc);
+            in[NA + r - R0] = ark_face_in(GEN ? ghzh[r] : P.D.gh[2], c.rho, c.w, c.p, c.rc, c.irc, wn[r].rho, wn[r].w, wn[r].p, wn[r].rc, wn[r].irc);
         }
         {
             const ArkPrim &a = wc[0], &b = wc[1];
-            in[2 * NA] = ark_face_in(ghy, a.rho, a.v, a.p, a.rc, a.irc, b.rho, b.v, b.p, b.rc, b.irc);
-            if (ROLE != 0) in[NF - 1] = ark_face_in(ghy, Bm.rho, Bm.v, Bm.p, Bm.rc, Bm.irc, a.rho, a.v, a.p, a.rc, a.irc);
+            in[2 * NA] = ark_face_in(GEN ? ghyi : ghy, a.rho, a.v, a.p, a.rc, a.irc, b.rho, b.v, b.p, b.rc, b.irc);
+            if (ROLE != 0) in[NF - 1] = ark_face_in(GEN ? ghyl : ghy, Bm.rho, Bm.v, Bm.p, Bm.rc, Bm.irc, a.rho, a.v, a.p, a.rc, a.irc);
         }
         ark_face_n<NF>(P.theta, in, out);
 #pragma unroll
@@ -452,7 +480,7 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         if (gy) fyu.S = M.FB[2 * NT + s + RX];
     }
     double Uc[2][5], Ut[2][5], Six[2] = {0, 0}, Siy[2] = {0, 0}, Siz[2] = {0, 0};
-    double usxh[2], pixh[2];
+    double usxh[2], pixh[2], Sxh[2] = {0, 0}, suS[2] = {0, 0};
 #pragma unroll
     for (int r = 0; r < 2; ++r) { for (int f = 0; f < 5; ++f) Uc[r][f] = Ut[r][f] = 0.0; usxh[r] = pixh[r] = 0.0; }
     {
@@ -465,7 +493,7 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
             const double* uc = M.UR + M.uq * 5 * NCOL + M.ca + r * RX;
             Uc[r][0] = wc[r].rho; Uc[r][1] = uc[NCOL]; Uc[r][2] = uc[2 * NCOL]; Uc[r][3] = uc[3 * NCOL]; Uc[r][4] = uc[4 * NCOL];
             usxh[r] = ark_xr(fx[r].us); pixh[r] = ark_xr(fx[r].pi);
-            if (gx) Six[r] = 0.5 * (fx[r].S + ark_xr(fx[r].S));   // S_i = (S_low + S_high)/2
+            if (gx) { Sxh[r] = ark_xr(fx[r].S); Six[r] = 0.5 * (fx[r].S + Sxh[r]); }   // S_i = (S_low + S_high)/2
         }
 #pragma unroll
         for (int r = R0; r <= R1; ++r) {
@@ -485,7 +513,14 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
             Ut[r][1] = GXY ? (Uc[r][1] - lam * (pixh[r] - fx[r].pi) + lam * Six[r]) : (Uc[r][1] - lam * (pixh[r] - fx[r].pi));
             Ut[r][2] = GXY ? (Uc[r][2] - lam * (yh[r]->pi - yl[r]->pi) + lam * Siy[r]) : (Uc[r][2] - lam * (yh[r]->pi - yl[r]->pi));
             Ut[r][3] = (Uc[r][3] - lam * (zhi[r].pi - M.zlo[r].pi) + lam * Siz[r]);
-            Ut[r][4] = (Uc[r][4] - lam * sdpu[r]);
+            if (eformB) {
+                // Appendix B (reading A24): (uS)_i = 1/2 (u* S at the high face + u* S at the low face), per axis
+                suS[r] = 0.5 * (usxh[r] * Sxh[r] + fx[r].us * fx[r].S) + 0.5 * (yh[r]->us * yh[r]->S + yl[r]->us * yl[r]->S)
+                       + 0.5 * (zhi[r].us * zhi[r].S + M.zlo[r].us * M.zlo[r].S);
+                Ut[r][4] = ((Uc[r][4] + lam * suS[r]) - lam * sdpu[r]);
+            } else {
+                Ut[r][4] = (Uc[r][4] - lam * sdpu[r]);
+            }
         }
 #pragma unroll
         for (int r = R0; r <= R1; ++r) {
@@ -556,8 +591,13 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
                 for (int f = 0; f < 5; ++f) { out[0][f] = acc[0][f] - lam * Gz[0][f]; out[1][f] = acc[1][f] - lam * Gz[1][f]; }
 #pragma unroll
                 for (int f = 0; f < 5; ++f) out[1][f] -= lam * fyh[f];
-                if (gy) out[1][4] += K.dt * P.g[1] * ark_neg_part(fyh[0]);
-                if (P.D.g_on[2]) { out[0][4] += K.dt * P.g[2] * ark_neg_part(Gz[0][0]); out[1][4] += K.dt * P.g[2] * ark_neg_part(Gz[1][0]); }
+                if (GEN) {
+                    if (wk && gy) out[1][4] += lam * M.ghyu_prev * ark_neg_part(fyh[0]);
+                    if (wk && P.D.g_on[2]) { out[0][4] += lam * M.ghz[0] * ark_neg_part(Gz[0][0]); out[1][4] += lam * M.ghz[1] * ark_neg_part(Gz[1][0]); }
+                } else {
+                    if (gy) out[1][4] += K.dt * P.g[1] * ark_neg_part(fyh[0]);
+                    if (P.D.g_on[2]) { out[0][4] += K.dt * P.g[2] * ark_neg_part(Gz[0][0]); out[1][4] += K.dt * P.g[2] * ark_neg_part(Gz[1][0]); }
+                }
 #pragma unroll
                 for (int r = 0; r < 2; ++r) {
                     if (M.inU[r]) {
@@ -626,7 +666,12 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
                 acc[r][1] = GXY ? (Uc[r][1] - lam * (Fh[r][1] - Fl[r][1]) + lam * Six[r]) + lam * Gz[r][1] : (Uc[r][1] - lam * (Fh[r][1] - Fl[r][1])) + lam * Gz[r][1];
                 acc[r][2] = GXY ? (Uc[r][2] - lam * (Fh[r][2] - Fl[r][2]) + lam * Siy[r]) + lam * Gz[r][2] : (Uc[r][2] - lam * (Fh[r][2] - Fl[r][2])) + lam * Gz[r][2];
                 acc[r][3] = (Uc[r][3] - lam * (Fh[r][3] - Fl[r][3])) + lam * Gz[r][3];
-                if (GXY) {
+                if (GEN) {
+                    double work = 0.0;                                  // (in units of lam)
+                    if (eformB) work = suS[r];
+                    else if (gx) work = ghxl[r] * ark_pos_part(Fl[r][0]) + ghxh[r] * ark_neg_part(Fh[r][0]);
+                    acc[r][4] = (Uc[r][4] - lam * (Fh[r][4] - Fl[r][4]) + lam * work) + lam * Gz[r][4];
+                } else if (GXY) {
                     double work = 0.0;
                     if (gx) work = P.g[0] * (ark_pos_part(Fl[r][0]) + ark_neg_part(Fh[r][0]));
                     acc[r][4] = (Uc[r][4] - lam * (Fh[r][4] - Fl[r][4]) + K.dt * work) + lam * Gz[r][4];
@@ -635,14 +680,16 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
                 }
                 if (P.D.g_on[2]) {
                     acc[r][3] += lam * Siz[r];
-                    acc[r][4] += K.dt * P.g[2] * ark_pos_part(Gz[r][0]);
+                    if (GEN) { if (wk) acc[r][4] += lam * M.ghz[r] * ark_pos_part(Gz[r][0]); }
+                    else acc[r][4] += K.dt * P.g[2] * ark_pos_part(Gz[r][0]);
                 }
             }
 #pragma unroll
             for (int f = 0; f < 5; ++f) { acc[0][f] -= lam * F[0][f]; acc[1][f] += lam * F[0][f]; }
-            if (gy) {
-                acc[0][4] += K.dt * P.g[1] * ark_neg_part(F[0][0]);
-                acc[1][4] += K.dt * P.g[1] * ark_pos_part(F[0][0]);
+            if (gy && wk) {
+                const double cy = GEN ? lam * ghyi : K.dt * P.g[1];
+                acc[0][4] += cy * ark_neg_part(F[0][0]);
+                acc[1][4] += cy * ark_pos_part(F[0][0]);
             }
             ark_tm_put5(tm + ARK_TM_AC(1), acc[1]);               // row b is complete but for its high-y / high-z faces
         }
@@ -660,7 +707,7 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         if (ROLE == 1) {
 #pragma unroll
             for (int f = 0; f < 5; ++f) acc[0][f] += lam * F[f];
-            if (gy) acc[0][4] += K.dt * P.g[1] * ark_pos_part(F[0]);
+            if (gy && wk) acc[0][4] += (GEN ? lam * ghyl : K.dt * P.g[1]) * ark_pos_part(F[0]);
             ark_tm_put5(tm + ARK_TM_AC(0), acc[0]);
         }
     }
@@ -674,21 +721,22 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     }
 #pragma unroll
     for (int r = R0; r <= R1; ++r) M.zlo[r] = zhi[r];
+    if (GEN) { M.ghz[0] = ghzh[0]; M.ghz[1] = ghzh[1]; M.ghyu_prev = ghyu; M.php += M.pstride; }
     M.tcur ^= 1;
     { const int t3 = M.uq; M.uq = M.un; M.un = M.unn; M.unn = t3; }
     { const int t2 = M.pc; M.pc = M.pn; M.pn = t2; }
 }
 
-template <bool VISC, bool GXY, int TX, int NW, int ROLE>
+template <bool VISC, bool GXY, bool GEN, int TX, int NW, int ROLE>
 ARK_DEV void ark_march3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VISC, TX, NW>& M) {
     int q = M.k0 - 1;
-    for (; q <= M.k0; ++q) ark_plane3<VISC, GXY, TX, NW, ROLE, false>(P, K, M, q);   // k0-1, k0
-    for (; q < M.k1; ++q) ark_plane3<VISC, GXY, TX, NW, ROLE, true>(P, K, M, q);     // k0+1 .. k1-1
-    for (; q <= M.k1; ++q) ark_plane3<VISC, GXY, TX, NW, ROLE, false>(P, K, M, q);   // k1
+    for (; q <= M.k0; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, false>(P, K, M, q);   // k0-1, k0
+    for (; q < M.k1; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, true>(P, K, M, q);     // k0+1 .. k1-1
+    for (; q <= M.k1; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, false>(P, K, M, q);   // k1
 }
 
 // prologue (planes k0-2, k0-1; k0 in flight) and plane loop of one row pair
-template <bool VISC, bool GXY, int TX, int NW, int ROLE>
+template <bool VISC, bool GXY, bool GEN, int TX, int NW, int ROLE>
 ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VISC, TX, NW>& M) {
     using C = ArkCfg3<VISC, TX, NW>;
     constexpr int RX = C::RX, NS = C::NS;
@@ -701,7 +749,16 @@ ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<
         wc0[r] = ark_march_prims3(P, M, M.ca + r * RX, 1);
         ark_tm_put_prim(M.tm + ARK_TM_PR(1, r), wm);              // plane k0-2 (the "q-1" slot of the first iteration)
         ark_tm_put_prim(M.tm + ARK_TM_PR(0, r), wc0[r]);          // plane k0-1
-        M.zlo[r] = ark_face(P.theta, P.D.gh[2], wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0[r].rho, wc0[r].w, wc0[r].p, wc0[r].rc, wc0[r].irc);
+        double ghz0 = P.D.gh[2];
+        if (GEN) {
+            if (P.phi) {                                  // M.php points at plane k0: planes k0-2, k0-1 of this column
+                const double phm = M.php[M.pho[1 + r] - 2 * M.pstride];
+                M.phc[r] = M.php[M.pho[1 + r] - M.pstride];
+                ghz0 = phm - M.phc[r];
+            }
+            M.ghz[r] = ghz0;
+        }
+        M.zlo[r] = ark_face(P.theta, ghz0, wm.rho, wm.w, wm.p, wm.rc, wm.irc, wc0[r].rho, wc0[r].w, wc0[r].p, wc0[r].rc, wc0[r].irc);
         if (ROLE == 1) {
             const double zero5[5] = {0, 0, 0, 0, 0};
             ark_tm_put5(M.tm + ARK_TM_TP(r), zero5);
@@ -720,7 +777,7 @@ ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<
         p[0] = wc0[0].u; p[NS] = wc0[0].v; p[2 * NS] = wc0[0].w;
     }
     __syncthreads();                                  // primitives of plane k0-1 visible to the neighbours
-    ark_march3<VISC, GXY, TX, NW, ROLE>(P, K, M);
+    ark_march3<VISC, GXY, GEN, TX, NW, ROLE>(P, K, M);
     ark_tm_wait_st();
 }
 
@@ -732,7 +789,7 @@ template <int N> ARK_DEV void ark_setmaxnreg_dec() {}
 template <int N> ARK_DEV void ark_setmaxnreg_inc() {}
 #endif
 
-template <bool VISC, bool GXY, int TX, int NW>
+template <bool VISC, bool GXY, bool GEN, int TX, int NW>
 ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin, double* __restrict__ Uout, double dt_value,
                               const double* __restrict__ dt_dev, double* __restrict__ rate_scratch, int zchunk, double* smem,
                               const void* tmap) {
@@ -787,6 +844,18 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
         const int lo = gi < P.nx ? gi : P.nx - 1, ljo = gja < P.ny ? gja : P.ny - 1;
         M.Ocur = Uout + (long long)(lo + ARK_XOFF) + (long long)P.px * (long long)(ljo + ARK_NG) + M.pstride * (long long)(P.offz + M.k0 - 2);
     }
+    M.php = nullptr;
+    M.phc[0] = M.phc[1] = M.ghz[0] = M.ghz[1] = M.ghyu_prev = 0.0;
+    M.pho[0] = M.pho[1] = M.pho[2] = M.pho[3] = 0;
+    if (GEN && P.phi) {
+        const int li = gi < P.nx + 2 ? gi : P.nx + 1;
+        for (int i = 0; i < 4; ++i) {
+            int gj = gja - 1 + i;
+            gj = gj < -ARK_NG ? -ARK_NG : (gj < P.ny + 2 ? gj : P.ny + 1);
+            M.pho[i] = P.px * (gj + ARK_NG);
+        }
+        M.php = P.phi + (li + ARK_XOFF) + M.pstride * (long long)(P.offz + M.k0);   // plane q+1 at q = k0-1
+    }
     M.tmap = tmap;
     M.tx = (int)(blockIdx.x * TX) - 2 + ARK_XOFF;
     M.ty = (int)(blockIdx.y * TY) - 2 + ARK_NG;
@@ -804,7 +873,9 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     ark_tm_fence_after_sync();
     tmem_base = *tm_slot;
     // TMEM scratch of this thread: lane quarter of the warp, column range of the warp within the quarter
-    M.tm = tmem_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)((warp >> 2) * ARK_TM_COLS);
+    // (warp-uniform by construction; the OR-reduction hands it to the compiler as a uniform-register value, so that
+    // every tcgen05.ld / st addresses tmem[UR + imm] without a per-instruction register -> uniform-register move)
+    M.tm = __reduce_or_sync(0xffffffffu, tmem_base + ((unsigned)(32 * (warp & 3)) << 16) + (unsigned)((warp >> 2) * ARK_TM_COLS));
 #else
     M.tm = 0; (void)tmem_base;
 #endif
@@ -818,8 +889,8 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
 
     if (warp < 4) {
         ark_setmaxnreg_dec<C::REG_RING>();
-        if (pair == 0)           ark_run_pair3<VISC, GXY, TX, NW, 0>(P, K, M);
-        else if (pair == NW - 1) ark_run_pair3<VISC, GXY, TX, NW, 2>(P, K, M);
+        if (pair == 0)           ark_run_pair3<VISC, GXY, GEN, TX, NW, 0>(P, K, M);
+        else if (pair == NW - 1) ark_run_pair3<VISC, GXY, GEN, TX, NW, 2>(P, K, M);
         else {
             // warps 2, 3: no rows; they only take part in the block barriers (1 after the prologue, 2 per plane)
             __syncthreads();
@@ -827,7 +898,7 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
         }
     } else {
         ark_setmaxnreg_inc<C::REG_TILE>();
-        ark_run_pair3<VISC, GXY, TX, NW, 1>(P, K, M);
+        ark_run_pair3<VISC, GXY, GEN, TX, NW, 1>(P, K, M);
     }
 
     if (rate_scratch) {
@@ -855,7 +926,7 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
 #endif
 }
 
-template <bool VISC, bool GXY, int TX, int NW>
+template <bool VISC, bool GXY, bool GEN, int TX, int NW>
 ARK_GLOBAL void
 #ifndef ARK_HOST_EMU
 __launch_bounds__(ArkCfg3<VISC, TX, NW>::NT, 1)
@@ -868,5 +939,5 @@ ark_k_step3(const ArkParams P, const double* __restrict__ Uin, double* __restric
 #else
     ARK_DYN_SMEM(smem);
 #endif
-    ark_step3d_pairs<VISC, GXY, TX, NW>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, zchunk, smem, ARK_TMAP_ARG);
+    ark_step3d_pairs<VISC, GXY, GEN, TX, NW>(P, Uin, Uout, dt_value, dt_dev, rate_scratch, zchunk, smem, ARK_TMAP_ARG);
 }

@@ -30,7 +30,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(build())
         _lib.emu_run.argtypes = ([C.c_int] * 3 + [C.c_double, C.c_double, _dp, C.c_double, C.c_double, C.c_int, _ip, _dp]
-                                 + [_dp] * 5 + [C.c_int, _dp, C.c_int, _dp, _dp, _dp])
+                                 + [_dp] * 5 + [C.c_int, _dp, C.c_int, _dp, _dp, _dp, C.c_int, _dp])
         _lib.emu_run.restype = C.c_int
     return _lib
 
@@ -40,7 +40,8 @@ def _p(a):
 
 
 def run(prm, U, dts, zchunk=0, want_padded=False):
-    """-> (U_new, rates_after_each_step, rate_of_initial_state[, padded ghost-filled initial state])"""
+    """-> (U_new, rates_after_each_step, rate_of_initial_state[, padded ghost-filled initial state]).
+    prm.get("energy_form") == 1 selects the Appendix-B energy update, prm.get("phi") an array-valued potential."""
     nx, ny, nz = prm["nx"], prm["ny"], prm["nz"]
     n = nx * ny * nz
     S = [np.zeros(n) if (a is None) else np.array(a, dtype=np.float64).reshape(-1).copy() for a in U]
@@ -52,9 +53,11 @@ def run(prm, U, dts, zchunk=0, want_padded=False):
     rate0 = np.zeros(1)
     nf = 5 if nz > 1 else 4
     padded = np.zeros(nf * (nx + 4) * (ny + 4) * ((nz + 4) if nz > 1 else 1)) if want_padded else None
+    phi = prm.get("phi")
+    phi = None if phi is None else np.ascontiguousarray(np.asarray(phi, dtype=np.float64).reshape(-1))
     lib().emu_run(nx, ny, nz, prm["dx"], prm["gamma"], _p(g), prm["mu"], prm["kappa"], prm["theta"],
                   bt.ctypes.data_as(_ip), _p(bv), *[_p(a) for a in S], len(dts), _p(dts), int(zchunk),
-                  _p(rates), _p(rate0), _p(padded))
+                  _p(rates), _p(rate0), _p(padded), int(prm.get("energy_form", 0)), _p(phi))
     out = (S, rates[:len(dts)], float(rate0[0]))
     if want_padded:
         shp = (nf, (nz + 4) if nz > 1 else 1, ny + 4, nx + 4)

@@ -38,15 +38,18 @@ void bc(const ArkParams& P, double* U, long long n) {
 
 template <int NDIM, bool VISC>
 void step(const ArkParams& P, const double* Uin, double* Uout, double dt, double* scratch, int zchunk, emu_dim3 grid) {
+    const bool gen = P.phi != nullptr || P.eform != 0;        // mirrors do_step in csrc/ark.cu
     if constexpr (NDIM == 3) {
         using C = ArkCfg3<VISC, ETX, ENW>;
         static_assert(C::TY == ETY, "emulation tile");
         const bool gxy = P.D.g_on[0] || P.D.g_on[1];
-        if (gxy) ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, true, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
-        else     ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, false, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
+        if (gen)      ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, true, true, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
+        else if (gxy) ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, true, false, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
+        else          ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step3<VISC, false, false, ETX, ENW>(P, Uin, Uout, dt, nullptr, scratch, zchunk); }, C::RX);
     } else {
         using C = ArkStepCfg<NDIM, VISC, ETX, ETY>;
-        ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch, zchunk); });
+        if (gen) ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, true, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch); });
+        else     ark_emu_launch(grid, C::NT, C::SMEM_BYTES, [&] { ark_k_step<NDIM, VISC, false, ETX, ETY>(P, Uin, Uout, dt, nullptr, scratch); });
     }
 }
 }  // namespace
@@ -58,10 +61,29 @@ extern "C" {
 // two-pass reduction of the initial state.  zchunk <= 0 picks nz (one chunk).
 int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, double mu, double kappa, int theta,
             const int* bt, const double* bv, double* rho, double* rhou, double* rhov, double* rhow, double* E,
-            int nsteps, const double* dts, int zchunk, double* rates_out, double* rate0_out, double* padded_out) {
-    const ArkParams P = make_params(nx, ny, nz, h, gamma, g, mu, kappa, theta, bt, bv);
+            int nsteps, const double* dts, int zchunk, double* rates_out, double* rate0_out, double* padded_out,
+            int eform, const double* phi) {
+    ArkParams P = make_params(nx, ny, nz, h, gamma, g, mu, kappa, theta, bt, bv);
+    P.eform = eform;
     std::vector<double> A((size_t)P.nf * P.fstride, 0.0), B((size_t)P.nf * P.fstride, 0.0);
-    std::vector<double> scratch(1 << 16, -1.0), result(2, 0.0);
+    std::vector<double> PhiPad;
+    if (phi) {
+        // mirrors ark_set_potential in csrc/ark.cu: pack, ghost sweeps x, y, z, all gravity terms on
+        PhiPad.assign((size_t)P.fstride, 0.0);
+        emu_dim3 gp; gp.x = (unsigned)(((long long)nx * ny * nz + 63) / 64);
+        ark_emu_launch(gp, 64, 0, [&] { ark_k_pack(P, PhiPad.data(), phi, 0); });
+        emu_dim3 g0; g0.x = (unsigned)(((long long)ny * nz + 63) / 64);
+        ark_emu_launch(g0, 64, 0, [&] { ark_k_phi_ghosts<0>(P, PhiPad.data()); });
+        emu_dim3 g1; g1.x = (unsigned)(((long long)(nx + 4) * nz + 63) / 64);
+        ark_emu_launch(g1, 64, 0, [&] { ark_k_phi_ghosts<1>(P, PhiPad.data()); });
+        if (P.ndim == 3) {
+            emu_dim3 g2; g2.x = (unsigned)(((long long)(nx + 4) * (ny + 4) + 63) / 64);
+            ark_emu_launch(g2, 64, 0, [&] { ark_k_phi_ghosts<2>(P, PhiPad.data()); });
+        }
+        P.phi = PhiPad.data();
+        for (int d = 0; d < P.ndim; ++d) P.D.g_on[d] = 1;
+    }
+    std::vector<double> scratch(1 << 16, -1.0), result(8, 0.0);   // [0] max rate, [1] dt, [3] sticky non-finite flag
     double* dense[5] = {rho, rhou, rhov, P.ndim == 3 ? rhow : E, E};
     const long long n = (long long)nx * ny * nz;
     emu_dim3 g1; g1.x = (unsigned)((n + 63) / 64);

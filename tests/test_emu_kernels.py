@@ -85,3 +85,54 @@ def test_emulated_nan_propagates_to_rate():
     U[4][0, 3, 5] = -5.0                       # negative pressure -> NaN sound speed
     _, _, rate0 = emu.run(prm, U, [])
     assert np.isnan(rate0)
+
+
+def _phi_field(nx, ny, nz, h, kind):
+    """A smooth non-linear potential at the cell centres (dense, x fastest)."""
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    x, y, z = (i + 0.5) * h, (j + 0.5) * h, (k + 0.5) * h
+    if kind == "periodic":
+        return 0.3 * np.cos(2 * np.pi * x / (nx * h)) * np.cos(2 * np.pi * y / (ny * h)) * (np.cos(2 * np.pi * z / (nz * h)) if nz > 1 else 1.0)
+    return 0.8 * y + 0.5 * y * y + 0.2 * np.sin(2 * np.pi * x / (nx * h)) + (0.6 * z + 0.3 * z * z * y if nz > 1 else 0.0)
+
+
+GEN_CASES = {
+    # SURVEY 8(f) row 4 (Appendix B, PAPER.md:514-546) and row 2 (array-valued potential, PAPER.md:55, :152)
+    "2d_appendix_b_const_g": lambda: (I.random_state(19, 11, 1, 31, mu=2e-3, kappa=3e-3, g=(0.3, -1.0, 0),
+                                                     bc_type=((PER, PER), (FIX, REF), (0, 0)), bc_value=((0, 0), (1.5, 0), (0, 0))), 1, None),
+    "2d_phi_periodic": lambda: (I.random_state(20, 10, 1, 32), 0, "periodic"),
+    "2d_phi_walls_appendix_b": lambda: (I.random_state(17, 12, 1, 33, mu=1e-3, kappa=2e-3,
+                                                       bc_type=((PER, PER), (REF, FIX), (0, 0)), bc_value=((0, 0), (0, 1.4), (0, 0))), 1, "walls"),
+    "3d_appendix_b_const_g": lambda: (I.random_state(12, 9, 10, 34, mu=2e-3, kappa=3e-3, g=(0, 0, -1.0),
+                                                     bc_type=((PER, PER), (PER, PER), (FIX, REF)), bc_value=((0, 0), (0, 0), (1.5, 0))), 1, None),
+    "3d_phi_periodic_inviscid": lambda: (I.random_state(12, 9, 7, 35), 0, "periodic"),
+    "3d_phi_walls_viscous": lambda: (I.random_state(10, 9, 9, 36, mu=1e-3, kappa=2e-3,
+                                                    bc_type=((PER, PER), (REF, REF), (FIX, REF)), bc_value=((0, 0), (0, 0), (1.5, 0))), 0, "walls"),
+    "3d_phi_walls_appendix_b": lambda: (I.random_state(9, 10, 8, 37, mu=1e-3, kappa=0.0,
+                                                       bc_type=((REF, REF), (PER, PER), (REF, REF))), 1, "walls"),
+}
+
+
+@pytest.mark.parametrize("name", sorted(GEN_CASES))
+def test_emulated_general_path_matches_oracle(name):
+    (prm, U), eform, kind = GEN_CASES[name]()
+    prm = dict(prm, energy_form=eform)
+    if kind is not None:
+        prm["phi"] = _phi_field(prm["nx"], prm["ny"], prm["nz"], prm["dx"], kind)
+    _compare(prm, U, 3)
+    if prm["nz"] > 1:
+        _compare(prm, U, 2, zchunk=4)
+
+
+def test_emulated_linear_potential_equals_constant_gravity():
+    """An array Phi = -g.x must give the constant-g result up to the rounding of the potential differences."""
+    prm, U = CASES["3d_all_walls_oblique_gravity"]()
+    nx, ny, nz, h = prm["nx"], prm["ny"], prm["nz"], prm["dx"]
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    g = prm["g"]
+    phi = -(g[0] * (i + 0.5) + g[1] * (j + 0.5) + g[2] * (k + 0.5)) * h
+    dts = O.run(prm, U, 3, cfl=0.4)[1]
+    A, _, _ = emu.run(prm, U, dts)
+    B, _, _ = emu.run(dict(prm, phi=phi), U, dts)
+    for f in range(5):
+        assert np.abs(A[f] - B[f]).max() <= 1e-13 * np.abs(A[f]).max(), f

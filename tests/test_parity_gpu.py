@@ -521,3 +521,90 @@ def test_second_workloads_at_full_size(B):
     s.close()
     assert d["max_speed"] < 1e-12, d
 
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# General path: Appendix-B energy update and array-valued potential
+# (PAPER.md:55, :152), through ark_set_energy_form / ark_set_potential
+# ---------------------------------------------------------------------------------------------------------------
+def _phi_field(nx, ny, nz, h, kind):
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    x, y, z = (i + 0.5) * h, (j + 0.5) * h, (k + 0.5) * h
+    if kind == "periodic":
+        return 0.3 * np.cos(2 * np.pi * x / (nx * h)) * np.cos(2 * np.pi * y / (ny * h)) * (np.cos(2 * np.pi * z / (nz * h)) if nz > 1 else 1.0)
+    return 0.8 * y + 0.5 * y * y + 0.2 * np.sin(2 * np.pi * x / (nx * h)) + (0.6 * z + 0.3 * z * z * y if nz > 1 else 0.0)
+
+
+GENERAL = {
+    "2d_appendix_b_walls_viscous": lambda: (I.random_state(67, 45, 1, 41, mu=2e-3, kappa=3e-3, g=(0.3, -1.0, 0),
+                                                           bc_type=((PER, PER), (FIX, REF), (0, 0)), bc_value=((0, 0), (2.5, 0), (0, 0))), 1, None),
+    "2d_phi_periodic": lambda: (I.random_state(70, 37, 1, 42), 0, "periodic"),
+    "2d_phi_walls_appendix_b": lambda: (I.random_state(50, 31, 1, 43, mu=1e-3, kappa=2e-3,
+                                                       bc_type=((PER, PER), (REF, FIX), (0, 0)), bc_value=((0, 0), (0, 2.4), (0, 0))), 1, "walls"),
+    "3d_appendix_b_walls_viscous": lambda: (I.random_state(37, 26, 40, 44, mu=2e-3, kappa=3e-3, g=(0, 0, -1.0),
+                                                           bc_type=((PER, PER), (PER, PER), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))), 1, None),
+    "3d_phi_periodic_inviscid": lambda: (I.random_state(45, 21, 19, 45), 0, "periodic"),
+    "3d_phi_walls_viscous": lambda: (I.random_state(41, 23, 30, 46, mu=1e-3, kappa=2e-3,
+                                                    bc_type=((PER, PER), (REF, REF), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))), 0, "walls"),
+    "3d_phi_all_walls_appendix_b": lambda: (I.random_state(33, 20, 18, 47, mu=1e-3, kappa=0.0,
+                                                           bc_type=((REF, REF), (REF, FIX), (REF, REF)), bc_value=((0, 0), (0, 3.5), (0, 0))), 1, "walls"),
+}
+
+
+@pytest.mark.parametrize("name", sorted(GENERAL))
+def test_parity_general_path(B, name):
+    """Appendix-B energy form and / or array-valued potential, O(1) random states, 5 steps, 1e-12 (as the random states)."""
+    (prm, U), eform, kind = GENERAL[name]()
+    prm = dict(prm, energy_form=eform)
+    if kind is not None:
+        prm["phi"] = _phi_field(prm["nx"], prm["ny"], prm["nz"], prm["dx"], kind)
+    ref, dts = O.run(prm, U, 5, cfl=0.4)
+    got = gpu_run(B, prm, U, dts)
+    err = rel_err(ref, got)
+    assert max(err) < 1e-12, (name, err)
+
+
+def test_general_path_config_shapes(B):
+    """10 steps at 1e-11 on the BASELINE recipes with the Appendix-B energy update (configs 1, 4) and with the constant
+    gravity of config 4 handed over as an array Phi = -g.x (the stratified column stays the paper's workload)."""
+    for prm, U in (I.config1_atmosphere(96), I.config4_rb3d(56)):
+        p2 = dict(prm, energy_form=1)
+        ref, dts = O.run(p2, U, 10, cfl=0.4)
+        got = gpu_run(B, p2, U, dts)
+        check_fields(ref, got, TOL, momentum_floor(p2, ref, dts), "appendix B")
+    prm, U = I.config4_rb3d(56)
+    n, h = prm["nx"], prm["dx"]
+    phi = np.broadcast_to((-prm["g"][2] * (np.arange(n) + 0.5) * h)[:, None, None], (n, n, n)).copy()
+    p3 = dict(prm, phi=phi)
+    ref, dts = O.run(p3, U, 10, cfl=0.4)
+    got = gpu_run(B, p3, U, dts)
+    check_fields(ref, got, TOL, momentum_floor(p3, ref, dts), "array potential")
+
+
+def test_array_potential_hydrostatic_rest_and_diagnostics(B):
+    """A column in discrete hydrostatic balance (relation (14)) with a NON-linear potential stays at rest
+    below 1e-12 on the GPU (well-balancing with an array-valued Phi), and ark_diagnostics uses Phi for the total energy."""
+    n, h = 64, 1.0 / 64
+    y = (np.arange(n) + 0.5) * h
+    Phic = y + 0.5 * y * y                                   # g grows with height
+    T = np.ones(n)
+    rho = np.zeros(n); rho[0] = 1.0
+    for j in range(n - 1):                                    # relation (14) with dphi of this potential (recipe A19)
+        d = Phic[j + 1] - Phic[j]
+        rho[j + 1] = rho[j] * (T[j] - 0.5 * d) / (T[j + 1] + 0.5 * d)
+    prm = I.make_params(48, n, 1, h, 1.4, g=(0.0, 0.0, 0.0), bc_type=((PER, PER), (REF, REF), (0, 0)))
+    R = np.broadcast_to(rho[:, None], (n, 48)).copy()
+    U = [R, np.zeros_like(R), np.zeros_like(R), None, R / 0.4]
+    phi = np.broadcast_to(Phic[:, None], (n, 48)).copy()
+    s = B.Solver(dict(prm, phi=phi))
+    s.set_state(to_dev(U))
+    d0 = s.diagnostics()
+    s.run(200, 0.4)
+    out = to_np(s.get_state())
+    d1 = s.diagnostics()
+    s.close()
+    vmax = max(np.abs(out[f] / out[0]).max() for f in (1, 2))
+    assert vmax < 1e-12, vmax
+    e_ref = float(((R / 0.4) + R * phi).sum() * h * h)
+    assert abs(d0["total_energy"] - e_ref) < 1e-12 * abs(e_ref)
+    assert abs(d1["total_energy"] - d0["total_energy"]) < 1e-12 * abs(e_ref)
