@@ -15,7 +15,7 @@ HEADERS = ["ark_device.cuh", "ark_step.cuh", "ark_step3d.cuh", os.path.join(".."
 # 3D: 28 outputs per row (32 lanes), ARK_NW3 row pairs per block (tile height 2 * NW3 - 4) on NW3 + 2 warps;
 # ARK_REG_RING / ARK_REG_TILE: setmaxnreg targets of the ring warpgroup and of the tile warpgroups (per scheduler:
 # 1 ring warp + 2 tile warps, REG_RING + 2 * REG_TILE <= 504: with 512 the allocation never completes)
-TILES = {"ARK_TX3": 28, "ARK_NW3": 10, "ARK_REG_RING": 88, "ARK_REG_TILE": 208, "ARK_TX2": 28, "ARK_TY2": 8,
+TILES = {"ARK_TX3": 28, "ARK_NW3": 10, "ARK_REG_RING": 72, "ARK_REG_TILE": 216, "ARK_TX2": 28, "ARK_TY2": 8,
          "ARK_TM_GRAN": 1}
 
 

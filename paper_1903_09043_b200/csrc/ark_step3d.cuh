@@ -18,8 +18,8 @@
 // rows are the outputs.  The role is a compile-time parameter of the whole plane loop and warp-uniform.
 //
 // Warp specialisation with register reallocation (setmaxnreg): the block has NW + 2 warps.  Warpgroup 0 (warps 0-3)
-// holds the two light ring pairs (warp 0: pair 0, warp 1: pair NW-1; warps 2, 3 only take part in the barriers) and
-// shrinks its register allowance; the tile pairs run on warps 4 .. NW+1 and grow theirs, so that every scheduler of
+// holds the two light ring pairs (warp 0: ring row 1, warp 1: ring row RY-2; warps 2, 3 compute the primitives of the
+// edge rows 0 and RY-1 for them) and shrinks its register allowance; the tile pairs run on warps 4 .. NW+1 and grow theirs, so that every scheduler of
 // the SM (warp w issues on scheduler w % 4) carries the same number of heavy tile warps.  The z pipeline of a column
 // (primitives of three planes, U~, running update, centred differences) is parked in TMEM between its uses.
 //
@@ -67,7 +67,8 @@ struct ArkCfg3 {
     static constexpr int TB_OFF = FB_OFF + 3 * NS;                   // [5][NS]       U~ of row b
     static constexpr int YB_OFF = TB_OFF + 5 * NS;                   // [5][NS]       flux through the low-y face of row a
     static constexpr int GB_OFF = YB_OFF + 5 * NS;                   // [4][NS]       dxv,dxu,dzv,dzw of row b (VISC)
-    static constexpr int RED_OFF = GB_OFF + (VISC ? 4 : 0) * NS;     // [32] block reduction of the rate
+    static constexpr int EB_OFF = GB_OFF + (VISC ? 4 : 0) * NS;      // [2][2][5][RX]  rho,v,p,rc,irc of the two edge rows, planes q, q+1
+    static constexpr int RED_OFF = EB_OFF + 20 * RX;                 // [32] block reduction of the rate
     static constexpr int MBAR_OFF = RED_OFF + 32;                    // [3] mbarriers of the UR slots
     static constexpr int SMEM_DOUBLES = MBAR_OFF + 4;
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
@@ -80,7 +81,7 @@ struct ArkCfg3 {
 
 template <bool VISC, int TX, int NW>
 struct ArkMarch3 {
-    double *UR, *PBb, *PBa, *FB, *TB, *YB, *GB;
+    double *UR, *PBb, *PBa, *FB, *TB, *YB, *GB, *EB;
     const double* Ucol[2];               // host emulation only: the two own columns of the input state
     const void* tmap;                    // tensor map of the input state (TMA tile loads of the UR ring)
     int tx, ty;                          // box origin in the padded array (columns, rows)
@@ -363,8 +364,8 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     ArkPrim wc[2], wn[2];
     double wm[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};
     ark_tm_wait_st();
-    ark_tm_get_prim(tm + ARK_TM_PR(tcur, 0), wc[0]);
-    ark_tm_get_prim(tm + ARK_TM_PR(tcur, 1), wc[1]);
+#pragma unroll
+    for (int r = R0; r <= R1; ++r) ark_tm_get_prim(tm + ARK_TM_PR(tcur, r), wc[r]);
     if (VISC) {
 #pragma unroll
         for (int r = R0; r <= R1; ++r) ark_tm_ld4(tm + ARK_TM_PR(tcur ^ 1, r), wm[r][0], wm[r][1], wm[r][2], wm[r][3]);
@@ -372,11 +373,15 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     if (STEADY || q + 2 <= M.k1 + 1) ark_ring_issue3(M, q + 2, M.unn);
     ark_ring_wait3(M, M.un);
     {
+        // (ring pairs: only the ring row; the primitives of their edge row come from the edge warps through EB)
         double U[2][5];
         const double* u = M.UR + M.un * 5 * NCOL + M.ca;
 #pragma unroll
-        for (int f = 0; f < 5; ++f) { U[0][f] = u[f * NCOL]; U[1][f] = u[f * NCOL + RX]; }
-        ark_prim_fast_n<2>(P, U, wn);
+        for (int f = 0; f < 5; ++f) {
+#pragma unroll
+            for (int r = R0; r <= R1; ++r) U[r][f] = u[f * NCOL + r * RX];
+        }
+        ark_prim_fast_n<NA>(P, U + R0, wn + R0);
     }
     if (ROLE != 2) {                                              // row b: all primitives, for the pair above
         double* p = M.PBb + M.pn * NP * NT + s;
@@ -402,6 +407,12 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         const double* n = M.PBb + M.pc * NP * NT + (s - RX);
         Bm.rho = n[0]; Bm.u = n[NT]; Bm.v = n[2 * NT]; Bm.w = n[3 * NT]; Bm.p = n[4 * NT]; Bm.rc = n[5 * NT]; Bm.irc = n[6 * NT];
         if (VISC) Bm.T = n[7 * NT];
+    }
+    if (ROLE != 1) {
+        // the edge row of a ring pair (row a of pair 0, row b of pair NW-1) only enters the (a|b) face
+        constexpr int RE = ROLE == 0 ? 0 : 1;
+        const double* e = M.EB + (M.pc * 2 + RE) * 5 * RX + (s % RX);
+        wc[RE].rho = e[0]; wc[RE].v = e[RX]; wc[RE].p = e[2 * RX]; wc[RE].rc = e[3 * RX]; wc[RE].irc = e[4 * RX];
     }
     {
         // faces in lock-step: x- and z+ of the active rows, low-y of row a (not for the low ring pair), (a|b)
@@ -452,8 +463,8 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         }
     }
     // plane q+1 is parked for the next iteration (its slot held plane q-1, which is in registers now)
-    ark_tm_put_prim(tm + ARK_TM_PR(tcur ^ 1, 0), wn[0]);
-    ark_tm_put_prim(tm + ARK_TM_PR(tcur ^ 1, 1), wn[1]);
+#pragma unroll
+    for (int r = R0; r <= R1; ++r) ark_tm_put_prim(tm + ARK_TM_PR(tcur ^ 1, r), wn[r]);
     if (VISC && ROLE == 1) {                                      // centred y differences of the two tile rows
         const double* n = M.PBa + M.pc * 3 * NT + (s + RX);      // row b+1 (pair above)
         dyu[0] = wc[1].u - Bm.u; dyv[0] = wc[1].v - Bm.v; dyw[0] = wc[1].w - Bm.w;
@@ -743,8 +754,9 @@ ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<
     ark_ring_wait3(M, 0);
     ark_ring_wait3(M, 1);
     ArkPrim wc0[2];
+    constexpr int R0 = ROLE == 0 ? 1 : 0, R1 = ROLE == 2 ? 0 : 1;   // active (ring / tile) rows of the pair
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
+    for (int r = R0; r <= R1; ++r) {
         const ArkPrim wm = ark_march_prims3(P, M, M.ca + r * RX, 0);
         wc0[r] = ark_march_prims3(P, M, M.ca + r * RX, 1);
         ark_tm_put_prim(M.tm + ARK_TM_PR(1, r), wm);              // plane k0-2 (the "q-1" slot of the first iteration)
@@ -781,6 +793,35 @@ ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<
     ark_tm_wait_st();
 }
 
+// Edge rows 0 and RY-1 of the region only provide primitives for one acoustic face each (the (a|b) face of the ring
+// pair next to them).  Warps 2 and 3 of warpgroup 0 compute them, one plane ahead like every other row, and hand
+// rho, v, p, rho c, 1/(rho c) to the ring warps through EB: the ring warps, which run alone on their schedulers next to
+// two tile warps and are on the critical path of every block barrier, carry one row instead of two.
+template <bool VISC, int TX, int NW>
+ARK_DEV void ark_edge_prims3(const ArkParams& P, const ArkMarch3<VISC, TX, NW>& M, int e, int uslot, int pslot) {
+    using C = ArkCfg3<VISC, TX, NW>;
+    const ArkPrim w = ark_march_prims3(P, M, M.ca + e * C::RX, uslot);
+    double* d = M.EB + (pslot * 2 + e) * 5 * C::RX + (M.s % C::RX);
+    d[0] = w.rho; d[C::RX] = w.v; d[2 * C::RX] = w.p; d[3 * C::RX] = w.rc; d[4 * C::RX] = w.irc;
+}
+
+template <bool VISC, int TX, int NW>
+ARK_DEV void ark_run_edge3(const ArkParams& P, ArkMarch3<VISC, TX, NW>& M, int e) {
+    ark_ring_wait3(M, 0);
+    ark_ring_wait3(M, 1);
+    ark_edge_prims3(P, M, e, 1, M.pc);                // plane k0-1
+    __syncthreads();
+    for (int q = M.k0 - 1; q <= M.k1; ++q) {
+        if (q + 2 <= M.k1 + 1) ark_ring_issue3(M, q + 2, M.unn);   // (a no-op on the GPU: thread 0 issues the TMA loads)
+        ark_ring_wait3(M, M.un);
+        ark_edge_prims3(P, M, e, M.un, M.pn);         // plane q+1
+        { const int t3 = M.uq; M.uq = M.un; M.un = M.unn; M.unn = t3; }
+        { const int t2 = M.pc; M.pc = M.pn; M.pn = t2; }
+        __syncthreads();
+        __syncthreads();
+    }
+}
+
 #ifndef ARK_HOST_EMU
 template <int N> ARK_DEV void ark_setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> ARK_DEV void ark_setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
@@ -803,12 +844,13 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     M.TB = smem + C::TB_OFF;
     M.YB = smem + C::YB_OFF;
     M.GB = smem + C::GB_OFF;
+    M.EB = smem + C::EB_OFF;
     ark_u64* red = (ark_u64*)(smem + C::RED_OFF);
     M.mbar = (unsigned long long*)(smem + C::MBAR_OFF);
 
     const int t = threadIdx.x;
     const int lane = t % RX, warp = t / RX, pair = C::pair_of_warp(warp);
-    const int prow = pair < 0 ? 0 : pair;                       // warps 2, 3 own no rows
+    const int prow = pair >= 0 ? pair : (warp == 2 ? 0 : NW - 1);   // warps 2, 3: the edge row of the low / high ring pair
     M.s = prow * RX + lane;
     M.ca = (2 * prow) * RX + lane;
     const int gi = blockIdx.x * TX - 2 + lane, gja = blockIdx.y * TY - 2 + 2 * prow;   // interior-based cell coordinates (row a)
@@ -891,11 +933,7 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
         ark_setmaxnreg_dec<C::REG_RING>();
         if (pair == 0)           ark_run_pair3<VISC, GXY, GEN, TX, NW, 0>(P, K, M);
         else if (pair == NW - 1) ark_run_pair3<VISC, GXY, GEN, TX, NW, 2>(P, K, M);
-        else {
-            // warps 2, 3: no rows; they only take part in the block barriers (1 after the prologue, 2 per plane)
-            __syncthreads();
-            for (int q = M.k0 - 1; q <= M.k1; ++q) { __syncthreads(); __syncthreads(); }
-        }
+        else                     ark_run_edge3<VISC, TX, NW>(P, M, warp == 2 ? 0 : 1);   // warps 2, 3: the edge rows
     } else {
         ark_setmaxnreg_inc<C::REG_TILE>();
         ark_run_pair3<VISC, GXY, GEN, TX, NW, 1>(P, K, M);
