@@ -304,6 +304,47 @@ def measure_workload(name, K, W, dev, local, world, dist, e2e=True):
     return out
 
 
+def measure_slab(name, K, W, dev, local, world, rank, dist):
+    """Opt-in `--decomp slab`: ONE global workload split along z over the ranks
+    (strong scaling), halo planes exchanged before every step (NCCL P2P over NVLink), dt = min over ranks.  Device-timed,
+    max over ranks; value = global cells * K / time."""
+    import torch
+    from paper_1903_09043_b200 import binding, inputs, slab
+    fn, n, bpc, _ = WORKLOADS[name]
+    k0, k1 = slab.partition(n, world)[rank]
+    prm, U = getattr(inputs, fn)(n, device=dev, box=((k0, k1), (0, n), (0, n)))
+    U = [a.reshape(-1).contiguous() for a in U]
+    s = slab.SlabSolver(binding, prm, rank, world, dist if world > 1 else None, device=dev)
+    s.set_state(U)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        s.step(s.compute_dt(CFL))
+    l0 = s.s.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(K):
+        s.step(s.compute_dt(CFL))
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = max_over_ranks(e0.elapsed_time(e1), dist, dev)
+    launches = s.s.launch_count() - l0
+    assert s.compute_dt(CFL) > 0
+    out = {"ncell": n ** 3, "bpc": bpc, "ms_total": ms_total, "launches": launches, "clocks": clocks,
+           "value": n ** 3 * K / (ms_total * 1e-3), "halo_bytes_sent_per_step_per_rank": s.bytes_per_exchange(),
+           "planes": [k0, k1], "grid": [n, n, n]}
+    s.close()
+    return out
+
+
 def roofline_objects(name, m, world, version, fp64_peak):
     """(hbm roofline, fp64 roofline) of one measured workload."""
     peak, peak_src = measured_peaks()
@@ -342,6 +383,25 @@ def run_ours(args):
     version = binding.version_string()
     W = max(args.warmup, 3)
     K = args.steps
+    if args.decomp == "slab":
+        m = measure_slab(args.workload, K, W, dev, local, world, rank, dist)
+        if rank == 0:
+            peak, peak_src = measured_peaks()
+            print(json.dumps({
+                "metric": METRIC, "value": m["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": m["ms_total"] / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "grid": m["grid"], "cfl": CFL, "parallelism": "slab decomposition along z, %d ranks" % world,
+                           "step": "min-all-reduce of dt + halo exchange (2 planes x 5 fields per neighbour, NCCL P2P) + ark_step per rank",
+                           "l2": "inputs larger than L2", "library": version},
+                "roofline": {"bound": "hbm", "kernel": "ark_k_step3", "achieved": m["bpc"] * m["value"] / world / 1e9, "peak": peak, "unit": "GB/s",
+                             "frac": m["bpc"] * m["value"] / world / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                             "note": "whole-step effective algorithmic bandwidth per GPU (exchange included)"},
+                "halo_bytes_sent_per_step_per_rank": m["halo_bytes_sent_per_step_per_rank"],
+                "gpu_launches": m["launches"], "clocks": m["clocks"]}))
+        if dist is not None:
+            dist.destroy_process_group()
+        return
     m = measure_workload(args.workload, K, W, dev, local, world, dist, e2e=not args.no_e2e)
     fp64_peak = binding.measure_fp64_peak()
     also = None
@@ -397,6 +457,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config5_512", choices=sorted(WORKLOADS))
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default, north_star: the path does not shard) or ONE workload split along z (slab.py)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (kernel tuning runs)")
     ap.add_argument("--no-also", action="store_true", help="skip the config4_256 measurement that rides along with config5_512")

@@ -42,7 +42,10 @@ enum { ARK_OK = 0, ARK_EINVAL = -1, ARK_ENOMEM = -2, ARK_ECUDA = -3, ARK_ENONFIN
 
 /* Boundary kinds (A9; PAPER.md:295 ghost zones, :378 reflecting + hydrostatic extrapolation,
  * :457 fixed temperature, :435 imposed temperature flux).  Periodic must be set on both sides of an axis. */
-enum { ARK_BC_PERIODIC = 0, ARK_BC_REFLECTING = 1, ARK_BC_FIXED_T_WALL = 2, ARK_BC_FLUX_WALL = 3 };
+enum { ARK_BC_PERIODIC = 0, ARK_BC_REFLECTING = 1, ARK_BC_FIXED_T_WALL = 2, ARK_BC_FLUX_WALL = 3,
+       /* ghost zones that hold a neighbouring sub-domain's cells (regular domain decomposition): z axis of 3D
+        * grids only; the library never fills them, the caller does with ark_set_halo before every ark_step */
+       ARK_BC_EXTERNAL = 4 };
 
 typedef struct {
     int type[3][2];     /* [axis x,y,z][lo,hi] */
@@ -116,6 +119,20 @@ int ark_set_energy_form(ark_solver*, int form);
  * to 88 B per cell update in 3D (64 -> 72 B in 2D).  Asynchronous on the stream.  Errors: ARK_EINVAL, ARK_ECUDA. */
 size_t ark_potential_bytes(int nx, int ny, int nz);
 int ark_set_potential(ark_solver*, const double* d_phi, void* d_buffer, size_t buffer_bytes);
+
+/* Slab decomposition along z (PAPER.md:295 "regular domain decomposition ... ghost-cell pattern", :303-307): a
+ * sub-domain is an ordinary solver whose z sides that face a neighbour are ARK_BC_EXTERNAL.  Before every step each
+ * sub-domain hands out the two interior planes next to such a side (ark_get_halo) and receives the neighbour's into its
+ * ghost planes (ark_set_halo); the time step is the minimum of the sub-domains' ark_compute_dt.  A halo is
+ * ark_halo_bytes() bytes of DEVICE memory: [field][2 planes][ny+4 rows][row pitch], i.e. padded planes WITH their x / y
+ * ghost cells (ark_get_halo runs the x and y ghost sweeps first; the following ark_step does not repeat them), so that the
+ * assembled result is bit-identical to the undivided domain.  side: 0 = low z, 1 = high z.  Both calls are asynchronous
+ * on the stream; the caller moves the buffers between devices (NCCL send/recv or peer copies over NVLink).  ark_run and
+ * array-valued potentials are not available on sub-domains.  Errors: ARK_EINVAL (2D solver, bad side, side not
+ * external), ARK_ECUDA. */
+size_t ark_halo_bytes(int nx, int ny, int nz);
+int ark_get_halo(ark_solver*, int side, double* d_buf);
+int ark_set_halo(ark_solver*, int side, const double* d_buf);
 
 /* Diagnostics of the current state as the paper reports them (PAPER.md:398-407 maximum velocity, :435 mean absolute
  * velocity, :14 conserved mass and total energy).  out (HOST, 6 doubles) = { max |u|, mean |u|, kinetic energy

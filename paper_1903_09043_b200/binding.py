@@ -10,13 +10,16 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libark_b200.so")
+# ARK_B200_LIBRARY selects another build of the same C ABI (the strict measuring build of reading A20, kernel tuning
+# variants); the default is the in-tree product library
+LIB_PATH = os.environ.get("ARK_B200_LIBRARY") or os.path.join(_HERE, "libark_b200.so")
 
 ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
 BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
            "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
+           "ark_halo_bytes", "ark_get_halo", "ark_set_halo",
            "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
 
@@ -66,6 +69,12 @@ def load():
     lib.ark_potential_bytes.restype = C.c_size_t
     lib.ark_set_potential.argtypes = [vp, dp, vp, C.c_size_t]
     lib.ark_set_potential.restype = ip
+    lib.ark_halo_bytes.argtypes = [ip, ip, ip]
+    lib.ark_halo_bytes.restype = C.c_size_t
+    lib.ark_get_halo.argtypes = [vp, ip, dp]
+    lib.ark_get_halo.restype = ip
+    lib.ark_set_halo.argtypes = [vp, ip, dp]
+    lib.ark_set_halo.restype = ip
     lib.ark_step_kernel_timing.argtypes = [vp, ip]
     lib.ark_step_kernel_timing.restype = ip
     lib.ark_step_kernel_time.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_int)]
@@ -205,6 +214,22 @@ class Solver:
         ptrs = [None if a is None else C.c_void_p(a.data_ptr()) for a in out]
         _check(self._lib.ark_debug_get_padded(self._h, *ptrs))
         return out
+
+    # ------------------------------------------------------------------ slab decomposition (ARK_BC_EXTERNAL sides)
+    def halo_doubles(self):
+        return int(self._lib.ark_halo_bytes(self.nx, self.ny, self.nz)) // 8
+
+    def get_halo(self, side, out=None):
+        """the two interior planes next to z side `side` (0 low, 1 high) with their x / y ghost cells -> CUDA tensor."""
+        if out is None:
+            out = torch.empty(self.halo_doubles(), dtype=torch.float64, device=self.device)
+        _check(self._lib.ark_get_halo(self._h, int(side), C.c_void_p(out.data_ptr())))
+        return out
+
+    def set_halo(self, side, buf):
+        if buf.dtype != torch.float64 or not buf.is_contiguous() or buf.numel() != self.halo_doubles() or buf.device.type != "cuda":
+            raise ValueError("halo must be a contiguous float64 CUDA tensor of %d elements" % self.halo_doubles())
+        _check(self._lib.ark_set_halo(self._h, int(side), C.c_void_p(buf.data_ptr())))
 
     # ------------------------------------------------------------------ time stepping
     def compute_dt(self, cfl):

@@ -28,6 +28,19 @@ def nvcc_cmd(out, extra=()):
             + [os.path.join(CSRC, s) for s in SOURCES])
 
 
+LIB_STRICT = os.path.join(HERE, "libark_b200_strict.so")
+
+
+def build_strict(force: bool = False) -> str:
+    """The same sources with -DARK_STRICT --fmad=false (IEEE division / square root, no FMA contraction): not the
+    product, a measuring instrument for reading A20 (tests/test_parity_gpu.py::test_strict_build_*)."""
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    if not force and os.path.exists(LIB_STRICT) and all(os.path.getmtime(LIB_STRICT) >= os.path.getmtime(d) for d in deps):
+        return LIB_STRICT
+    subprocess.run(nvcc_cmd(LIB_STRICT, ["-DARK_STRICT=1", "--fmad=false"]), check=True)
+    return LIB_STRICT
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
@@ -39,3 +52,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--strict" in sys.argv:
+        print(build_strict(force="--force" in sys.argv))

@@ -85,6 +85,7 @@ struct ark_solver {
     cudaStream_t stream;
     int rate_slots;         // >0: scratch[0..rate_slots) holds the per-block rates of the CURRENT state
     bool xghost_valid;      // 3D, periodic x: the step kernel already wrote the x ghost columns of the current state
+    bool xyghost_valid;     // the x and y ghost sweeps already ran on the current state (ark_get_halo)
     dim3 step_grid;
     int zchunk;
     long long launches;
@@ -162,8 +163,10 @@ int launch_step2(ark_solver* s, double dt, const double* dt_dev) {
     return ARK_OK;
 }
 
-int launch_bc(ark_solver* s, double* U) {
+// x and y sweeps of the ghost fill (interior z range); the z sweep covers the extended x, y range afterwards
+int launch_bc_xy(ark_solver* s, double* U) {
     const ArkParams& P = s->P;
+    if (s->xyghost_valid) return ARK_OK;
     if (P.bc[0][0] == ARK_BCK_PERIODIC) {
         // (3D: the fused step kernel writes the periodic x ghost columns of the state it produces; the sweep is only
         // needed for a state that came from outside)
@@ -182,7 +185,15 @@ int launch_bc(ark_solver* s, double* U) {
         ark_k_bc<1><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
         s->launches++;
     }
-    if (P.ndim == 3) {
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+int launch_bc(ark_solver* s, double* U) {
+    const ArkParams& P = s->P;
+    const int rc = launch_bc_xy(s, U);
+    if (rc != ARK_OK) return rc;
+    if (P.ndim == 3 && !(P.bc[2][0] == ARK_BCK_EXTERNAL && P.bc[2][1] == ARK_BCK_EXTERNAL)) {
         const long long n = 2LL * (P.nx + 2 * ARK_NG) * (P.ny + 2 * ARK_NG);
         ark_k_bc<2><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
         s->launches++;
@@ -248,6 +259,7 @@ int do_step(ark_solver* s, double dt, const double* dt_dev) {
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
     s->xghost_valid = s->P.ndim == 3 && s->P.bc[0][0] == ARK_BCK_PERIODIC;
+    s->xyghost_valid = false;
     s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
     return ARK_OK;
 }
@@ -339,8 +351,10 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     for (int d = 0; d < ndim; ++d) {
         for (int sd = 0; sd < 2; ++sd) {
             const int t = bc->type[d][sd];
-            if (t != ARK_BC_PERIODIC && t != ARK_BC_REFLECTING && t != ARK_BC_FIXED_T_WALL && t != ARK_BC_FLUX_WALL)
+            if (t != ARK_BC_PERIODIC && t != ARK_BC_REFLECTING && t != ARK_BC_FIXED_T_WALL && t != ARK_BC_FLUX_WALL && t != ARK_BC_EXTERNAL)
                 return fail(ARK_EINVAL, "ark_create: unknown boundary kind%s");
+            if (t == ARK_BC_EXTERNAL && !(ndim == 3 && d == 2))
+                return fail(ARK_EINVAL, "ark_create: ARK_BC_EXTERNAL (slab decomposition) exists on the z axis of 3D grids only%s");
             if (t == ARK_BC_FLUX_WALL && !(kappa > 0.0))
                 return fail(ARK_EINVAL, "ark_create: an imposed-flux wall needs kappa > 0%s");
             if (t == ARK_BC_FIXED_T_WALL && !(bc->value[d][sd] > 0.0))
@@ -456,6 +470,7 @@ int ark_set_state(ark_solver* s, const double* rho, const double* rhou, const do
     ARK_CUDA(cudaGetLastError());
     s->rate_slots = 0;
     s->xghost_valid = false;
+    s->xyghost_valid = false;
     return ARK_OK;
 }
 
@@ -488,6 +503,7 @@ int ark_set_state_host(ark_solver* s, const double* rho, const double* rhou, con
     ARK_CUDA(cudaStreamSynchronize(s->stream));
     s->rate_slots = 0;
     s->xghost_valid = false;
+    s->xyghost_valid = false;
     return ARK_OK;
 }
 
@@ -585,6 +601,8 @@ int run_pairs_graph(ark_solver* s, int npairs, double cfl, double* dt_log) {
 int ark_run(ark_solver* s, int nsteps, double cfl, double* dts_out) {
     if (!s || nsteps < 0 || !(cfl > 0.0)) return fail(ARK_EINVAL, "ark_run: bad argument%s");
     ARK_ON_DEVICE(s);
+    if (s->P.ndim == 3 && (s->P.bc[2][0] == ARK_BCK_EXTERNAL || s->P.bc[2][1] == ARK_BCK_EXTERNAL))
+        return fail(ARK_EINVAL, "ark_run: a sub-domain with external ghost planes needs a halo exchange before every step%s");
     if (dts_out && nsteps > DTLOG_MAX) return fail(ARK_EINVAL, "ark_run: at most %s%lld steps when dts_out is given", "", (long long)DTLOG_MAX);
     double* dt_log = dts_out ? s->dtlog : nullptr;
     // result[3]: sticky "a rate was not finite and positive" flag of pass 2; result[4]: log counter
@@ -651,6 +669,8 @@ int ark_set_potential(ark_solver* s, const double* d_phi, void* d_buffer, size_t
     ARK_ON_DEVICE(s);
     ArkParams& P = s->P;
     if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    if (d_phi && P.ndim == 3 && (P.bc[2][0] == ARK_BCK_EXTERNAL || P.bc[2][1] == ARK_BCK_EXTERNAL))
+        return fail(ARK_EINVAL, "ark_set_potential: not available on a sub-domain with external ghost planes%s");
     if (!d_phi) {                                   // back to the constant gravity vector of ark_create
         P.phi = nullptr;
         ark_fill_derived(P);
@@ -673,6 +693,41 @@ int ark_set_potential(ark_solver* s, const double* d_phi, void* d_buffer, size_t
     ARK_CUDA(cudaGetLastError());
     P.phi = pad;
     for (int d = 0; d < P.ndim; ++d) P.D.g_on[d] = 1;          // every axis carries gravity terms now
+    return ARK_OK;
+}
+
+size_t ark_halo_bytes(int nx, int ny, int nz) {
+    if (!supported_grid(nx, ny, nz) || nz == 1) return 0;
+    const Layout L = make_layout(nx, ny, nz);
+    return (size_t)L.nf * ARK_NG * L.px * L.py * sizeof(double);
+}
+
+int ark_get_halo(ark_solver* s, int side, double* d_buf) {
+    if (!s || !d_buf || (side != 0 && side != 1) || s->P.ndim != 3) return fail(ARK_EINVAL, "ark_get_halo: bad argument (3D solvers only)%s");
+    ARK_ON_DEVICE(s);
+    // the planes travel with their x / y ghost cells: those sweeps run now (and are skipped by the next ark_step)
+    const int rc = launch_bc_xy(s, s->U[s->cur]);
+    if (rc != ARK_OK) return rc;
+    s->xyghost_valid = true;
+    const ArkParams& P = s->P;
+    const size_t plane = (size_t)P.px * P.py, chunk = ARK_NG * plane;
+    const int k0 = side == 0 ? 0 : P.nz - ARK_NG;                    // the two interior planes next to that side
+    for (int f = 0; f < P.nf; ++f)
+        ARK_CUDA(cudaMemcpyAsync(d_buf + f * chunk, s->U[s->cur] + f * P.fstride + (size_t)(k0 + P.offz) * plane, chunk * sizeof(double),
+                                 cudaMemcpyDeviceToDevice, s->stream));
+    return ARK_OK;
+}
+
+int ark_set_halo(ark_solver* s, int side, const double* d_buf) {
+    if (!s || !d_buf || (side != 0 && side != 1) || s->P.ndim != 3) return fail(ARK_EINVAL, "ark_set_halo: bad argument (3D solvers only)%s");
+    ARK_ON_DEVICE(s);
+    if (s->P.bc[2][side] != ARK_BCK_EXTERNAL) return fail(ARK_EINVAL, "ark_set_halo: that side is not ARK_BC_EXTERNAL%s");
+    const ArkParams& P = s->P;
+    const size_t plane = (size_t)P.px * P.py, chunk = ARK_NG * plane;
+    const int k0 = side == 0 ? -ARK_NG : P.nz;                       // the two ghost planes of that side
+    for (int f = 0; f < P.nf; ++f)
+        ARK_CUDA(cudaMemcpyAsync(s->U[s->cur] + f * P.fstride + (size_t)(k0 + P.offz) * plane, d_buf + f * chunk, chunk * sizeof(double),
+                                 cudaMemcpyDeviceToDevice, s->stream));
     return ARK_OK;
 }
 

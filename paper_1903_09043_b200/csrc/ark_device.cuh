@@ -28,7 +28,7 @@
 #define ARK_NG 2             // ghost layers (A9)
 #define ARK_XOFF 4           // x index of interior cell 0 inside a padded row (>= ARK_NG)
 
-enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2, ARK_BCK_FLUX = 3 };
+enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2, ARK_BCK_FLUX = 3, ARK_BCK_EXTERNAL = 4 };
 
 // Coefficients of the dissipative face flux (see ark_visc_face in ark_step.cuh).
 struct ArkViscCoef { double cn, ct, c43, c23t, kh; };
@@ -93,8 +93,13 @@ ARK_DEV ark_u64 ark_umax(ark_u64 a, ark_u64 b) { return a > b ? a : b; }
 // arguments in [2^-20, 2^21): 1.11e-16 (rcp), 1.38e-16 (rsqrt), i.e. <= 1.25 x 2^-53 -- against ~10 fp64
 // instructions plus a slow-path call for the IEEE division.
 // ------------------------------------------------------------------------------------------------
+// ARK_STRICT (libark_b200_strict.so, built with --fmad=false): IEEE division and square root instead, so that the
+// kernels' arithmetic differs from a plain evaluation only in what the source itself reorders (reading A20 on hardware).
+#if defined(ARK_HOST_EMU) || defined(ARK_STRICT)
+#define ARK_IEEE_RCP 1
+#endif
 ARK_DEV double ark_rcp(double x) {
-#ifndef ARK_HOST_EMU
+#ifndef ARK_IEEE_RCP
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     double e = fma(-x, y, 1.0);
@@ -106,13 +111,13 @@ ARK_DEV double ark_rcp(double x) {
 }
 
 ARK_DEV double ark_rsqrt(double x) {
-#ifndef ARK_HOST_EMU
+#ifndef ARK_IEEE_RCP
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double e = fma(-x * y, y, 1.0);              // 1 - x y^2
     return fma(y * e, fma(0.375, e, 0.5), y);          // y (1 + e/2 + 3 e^2/8): error ~ seed^3
 #else
-    return 1.0 / std::sqrt(x);
+    return 1.0 / sqrt(x);
 #endif
 }
 
@@ -266,7 +271,11 @@ ARK_DEV ArkPrim ark_prim(const ArkParams& P, double rho, double mx, double my, d
     const double ke = 0.5 * (mx * q.u + my * q.v + mz * q.w);
     q.p = P.gm1 * (E - ke);
     const double gpr = P.gamma * q.p * rho;        // (rho c)^2
+#ifdef ARK_STRICT
+    q.irc = 1.0 / sqrt(gpr);
+#else
     q.irc = rsqrt(gpr);
+#endif
     q.rc = gpr * q.irc;
     q.T = q.p * rinv;
     return q;
@@ -361,6 +370,7 @@ ARK_GLOBAL void ark_k_unpack_padded(ArkParams P, const double* __restrict__ U, d
 //   periodic: copy.   reflecting wall: u_n -> -u_n, T_g = T_src.
 //   fixed-T no-slip wall: u -> -u (all components), T_g = 2 T_w - T_src.
 //   imposed-flux wall (A22): u_n -> -u_n, T_g = T_src + (2l-1) F h / kappa (F = heat flux entering).
+//   external (ghost zones that hold the neighbouring sub-domain's cells): left as the caller set them.
 //   rho_g from the discrete hydrostatic relation (14), PAPER.md:237:
 //       p_g - p_prev = 1/2 (rho_prev + rho_g) delta,  delta = Phi_prev - Phi_g = -+ g_d h,  p_g = rho_g T_g
 //       (with an array-valued potential, P.phi: the difference of its padded values).
@@ -386,6 +396,7 @@ ARK_GLOBAL void ark_k_bc(ArkParams P, double* __restrict__ U) {
         else                { c[0] = a; c[1] = b; c[2] = 0; }
         const long long base = ark_idx(P, c[0], c[1], c[2]);     // index of interior cell 0 along AXIS
         const int type = P.bc[AXIS][side];
+        if (type == ARK_BCK_EXTERNAL) continue;                   // ghost planes supplied by the caller (slab decomposition, ark_set_halo)
         for (int l = 1; l <= ARK_NG; ++l) {
             const int ig = side == 0 ? -l : n - 1 + l;
             const long long jg = base + ig * sd;

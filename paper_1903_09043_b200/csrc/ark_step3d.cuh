@@ -188,7 +188,7 @@ ARK_DEV void ark_face_flux(double* F, bool left, const double* TL, const double*
 // ------------------------------------------------------------------------------------------------------------
 template <int N>
 ARK_DEV void ark_rcp_n(const double* x, double* r) {
-#ifndef ARK_HOST_EMU
+#ifndef ARK_IEEE_RCP
     double y[N], e[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y[i]) : "d"(x[i]));
@@ -205,7 +205,7 @@ ARK_DEV void ark_rcp_n(const double* x, double* r) {
 
 template <int N>
 ARK_DEV void ark_rsqrt_n(const double* x, double* r) {
-#ifndef ARK_HOST_EMU
+#ifndef ARK_IEEE_RCP
     double y[N], e[N], t[N];
 #pragma unroll
     for (int i = 0; i < N; ++i) asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y[i]) : "d"(x[i]));
@@ -220,7 +220,7 @@ ARK_DEV void ark_rsqrt_n(const double* x, double* r) {
 #pragma unroll
     for (int i = 0; i < N; ++i) r[i] = fma(e[i], t[i], y[i]);
 #else
-    for (int i = 0; i < N; ++i) r[i] = 1.0 / std::sqrt(x[i]);
+    for (int i = 0; i < N; ++i) r[i] = 1.0 / sqrt(x[i]);
 #endif
 }
 
