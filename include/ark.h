@@ -140,6 +140,15 @@ int ark_set_halo(ark_solver*, int side, const double* d_buf);
  * at the cell centres and dV = dx^ndim.  Two-pass reduction without atomics (bit-reproducible); synchronises. */
 int ark_diagnostics(ark_solver*, double* out);
 
+/* Kinetic-energy power spectrum of the horizontal middle plane (Fig. 11; reading A26): plane k = nz/2,
+ * w_c = sqrt(rho) u_c, w^_c(kx,ky) = 1/(nx ny) sum w_c exp(-2 pi i (kx i/nx + ky j/ny)); out[kappa] = sum over the shell
+ * floor(|k~| + 1/2) == kappa (signed wavenumbers) of 1/2 sum_c |w^_c|^2, kappa = 0 .. nbins-1, so that sum_kappa
+ * out[kappa] = mean of 1/2 rho |u|^2 over the plane.  out: HOST, nbins = ark_ke_spectrum_bins(nx, ny) doubles.  3D grids
+ * with nz >= 8 (the scratch lives in the library's staging field, which ark_set/get_state_host also use).  Plain DFT with
+ * fixed summation order (bit-reproducible).  Synchronises the stream.  Errors: ARK_EINVAL, ARK_ECUDA. */
+int ark_ke_spectrum_bins(int nx, int ny);
+int ark_ke_spectrum(ark_solver*, double* out, int nbins);
+
 /* Ghost fill only, then copy the PADDED current state ((nx+4)*(ny+4)*(nz+4 or 1) per field, x fastest)
  * to device arrays: test hook for the boundary kernel.  Asynchronous. */
 int ark_debug_get_padded(ark_solver*, double* rho, double* rhou, double* rhov, double* rhow, double* E);

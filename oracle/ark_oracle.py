@@ -128,3 +128,25 @@ def diagnostics(p, U):
 
 def K():
     return lib().oracle_K()
+
+
+def ke_spectrum(p, U):
+    """Kinetic-energy power spectrum of the horizontal middle plane (Fig. 11; the paper prints no
+    formula: reading A26 of DESIGN.md).  Plane k = nz // 2, w_c = sqrt(rho) u_c; w^_c = fft2(w_c) / (nx ny) (library FFT
+    as the plain definition of the discrete Fourier transform); E[kappa] = sum over the shell floor(|k~| + 1/2) == kappa
+    (signed integer wavenumbers) of 1/2 sum_c |w^_c|^2.  Pinned by Parseval (sum E = plane mean of 1/2 rho |u|^2), a single
+    Fourier mode in closed form and a brute-force DFT (tests/test_oracle_pins.py)."""
+    nx, ny, nz = int(p["nx"]), int(p["ny"]), int(p["nz"])
+    S = [a.reshape(nz, ny, nx) for a in _state(p, U)]
+    k = nz // 2
+    rho = S[0][k]
+    power = np.zeros((ny, nx))
+    for c in (1, 2, 3):
+        w = S[c][k] / np.sqrt(rho)
+        W = np.fft.fft2(w) / (nx * ny)
+        power += 0.5 * (W.real ** 2 + W.imag ** 2)
+    kx = np.fft.fftfreq(nx, 1.0 / nx)[None, :]
+    ky = np.fft.fftfreq(ny, 1.0 / ny)[:, None]
+    shell = np.floor(np.sqrt(kx * kx + ky * ky) + 0.5).astype(np.int64)
+    nb = int(np.floor(np.sqrt((nx // 2) ** 2 + (ny // 2) ** 2) + 0.5)) + 1
+    return np.bincount(shell.reshape(-1), weights=power.reshape(-1), minlength=nb)[:nb]

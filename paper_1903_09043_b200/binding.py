@@ -19,7 +19,7 @@ BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
            "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
-           "ark_halo_bytes", "ark_get_halo", "ark_set_halo",
+           "ark_halo_bytes", "ark_get_halo", "ark_set_halo", "ark_ke_spectrum_bins", "ark_ke_spectrum",
            "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
 
@@ -69,6 +69,10 @@ def load():
     lib.ark_potential_bytes.restype = C.c_size_t
     lib.ark_set_potential.argtypes = [vp, dp, vp, C.c_size_t]
     lib.ark_set_potential.restype = ip
+    lib.ark_ke_spectrum_bins.argtypes = [ip, ip]
+    lib.ark_ke_spectrum_bins.restype = ip
+    lib.ark_ke_spectrum.argtypes = [vp, C.POINTER(C.c_double), ip]
+    lib.ark_ke_spectrum.restype = ip
     lib.ark_halo_bytes.argtypes = [ip, ip, ip]
     lib.ark_halo_bytes.restype = C.c_size_t
     lib.ark_get_halo.argtypes = [vp, ip, dp]
@@ -253,6 +257,13 @@ class Solver:
         buf = (C.c_double * 6)()
         _check(self._lib.ark_diagnostics(self._h, buf))
         return dict(zip(("max_speed", "mean_speed", "kinetic_energy", "max_mach", "mass", "total_energy"), list(buf)))
+
+    def ke_spectrum(self):
+        """kinetic-energy power spectrum of the horizontal middle plane -> list over shells kappa."""
+        nb = int(self._lib.ark_ke_spectrum_bins(self.nx, self.ny))
+        buf = (C.c_double * nb)()
+        _check(self._lib.ark_ke_spectrum(self._h, buf, nb))
+        return list(buf)
 
     def step_kernel_timing(self, enable=True):
         _check(self._lib.ark_step_kernel_timing(self._h, int(bool(enable))))

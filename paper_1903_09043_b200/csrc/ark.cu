@@ -731,6 +731,37 @@ int ark_set_halo(ark_solver* s, int side, const double* d_buf) {
     return ARK_OK;
 }
 
+int ark_ke_spectrum_bins(int nx, int ny) {
+    if (nx < 4 || ny < 4) return 0;
+    return (int)std::floor(std::sqrt((double)(nx / 2) * (nx / 2) + (double)(ny / 2) * (ny / 2)) + 0.5) + 1;
+}
+
+int ark_ke_spectrum(ark_solver* s, double* out, int nbins) {
+    if (!s || !out) return fail(ARK_EINVAL, "ark_ke_spectrum: NULL argument%s");
+    ARK_ON_DEVICE(s);
+    const ArkParams& P = s->P;
+    if (P.ndim != 3 || P.nz < 8) return fail(ARK_EINVAL, "ark_ke_spectrum: needs a 3D grid with nz >= 8 (scratch lives in the staging field)%s");
+    if (nbins != ark_ke_spectrum_bins(P.nx, P.ny) || nbins > 4096) return fail(ARK_EINVAL, "ark_ke_spectrum: nbins must be ark_ke_spectrum_bins(nx, ny)%s");
+    // scratch inside the dense staging field (nx*ny*nz doubles): A 6 nx ny | Pw nx ny | twiddles 2 nx + 2 ny | E nbins
+    const long long n = (long long)P.nx * P.ny;
+    if (7 * n + 2 * (P.nx + P.ny) + nbins > n * P.nz) return fail(ARK_EINVAL, "ark_ke_spectrum: grid too thin for the scratch%s");
+    double* A = s->stage;
+    double* Pw = A + 6 * n;
+    double* twx = Pw + n;
+    double* twy = twx + 2 * P.nx;
+    double* E = twy + 2 * P.ny;
+    ark_k_spec_twiddle<<<grid_for(P.nx, 128), 128, 0, s->stream>>>(twx, P.nx);
+    ark_k_spec_twiddle<<<grid_for(P.ny, 128), 128, 0, s->stream>>>(twy, P.ny);
+    ark_k_spec_rows<<<grid_for(n, 128, 148 * 16), 128, 0, s->stream>>>(P, s->U[s->cur], P.nz / 2, twx, A);
+    ark_k_spec_cols<<<grid_for(n, 128, 148 * 16), 128, 0, s->stream>>>(P, A, twy, Pw);
+    ark_k_spec_bins<<<nbins, 256, 0, s->stream>>>(P, Pw, E);
+    s->launches += 5;
+    ARK_CUDA(cudaGetLastError());
+    ARK_CUDA(cudaMemcpyAsync(out, E, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    ARK_CUDA(cudaStreamSynchronize(s->stream));
+    return ARK_OK;
+}
+
 int ark_measure_fp64_peak(double* tinstr_per_s, void* cuda_stream) {
     if (!tinstr_per_s) return fail(ARK_EINVAL, "ark_measure_fp64_peak: NULL argument%s");
     cudaStream_t st = (cudaStream_t)cuda_stream;

@@ -630,6 +630,88 @@ ARK_GLOBAL void ark_k_cfl_pass2(const double* __restrict__ scratch, int nvals, d
 }
 
 // ------------------------------------------------------------------------------------------------
+// Kinetic-energy power spectrum of the horizontal middle plane (Fig. 11; the paper prints no formula:
+// reading A26 of DESIGN.md).  Plane k = nz/2, w_c = sqrt(rho) u_c = m_c / sqrt(rho), c = x, y, z;
+//   w^_c(kx,ky) = 1/(nx ny) sum_{i,j} w_c(i,j) exp(-2 pi i (kx i / nx + ky j / ny)),
+//   E(kappa) = sum over (kx,ky) with floor(sqrt(kx~^2 + ky~^2) + 1/2) == kappa of 1/2 sum_c |w^_c|^2   (kx~, ky~ signed),
+// so that sum_kappa E(kappa) = mean over the plane of 1/2 rho |u|^2 (Parseval).  A plain separable DFT with tabulated
+// twiddles (exact index arithmetic (kx i) mod nx, sincospi): O(n^3) per plane, milliseconds at 512^2, every sum in a
+// fixed order (bit-reproducible, no atomics).  Diagnostic, not part of the time step.
+// ------------------------------------------------------------------------------------------------
+#ifndef ARK_HOST_EMU
+ARK_GLOBAL void ark_k_spec_twiddle(double* __restrict__ tw, int n) {       // tw[2t], tw[2t+1] = cos, sin (2 pi t / n)
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x) {
+        double sn, cs;
+        sincospi(2.0 * (double)t / (double)n, &sn, &cs);
+        tw[2 * t] = cs; tw[2 * t + 1] = sn;
+    }
+}
+// A[c][j][kx] = sum_i w_c(i,j) exp(-2 pi i kx i / nx)   (complex, interleaved), one thread per (j, kx)
+ARK_GLOBAL void ark_k_spec_rows(ArkParams P, const double* __restrict__ U, int kplane, const double* __restrict__ twx, double* __restrict__ A) {
+    const long long n = (long long)P.nx * P.ny;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(s % P.nx), j = (int)(s / P.nx);
+        const double* row = U + ark_idx(P, 0, j, kplane);
+        double re[3] = {0, 0, 0}, im[3] = {0, 0, 0};
+        int t = 0;
+        for (int i = 0; i < P.nx; ++i) {
+            const double isr = 1.0 / sqrt(row[i]);
+            const double cs = twx[2 * t], sn = twx[2 * t + 1];
+            for (int c = 0; c < 3; ++c) {
+                const double w = row[(c + 1) * P.fstride + i] * isr;
+                re[c] += w * cs; im[c] -= w * sn;
+            }
+            t += kx; if (t >= P.nx) t -= P.nx;
+        }
+        for (int c = 0; c < 3; ++c) { A[2 * (c * n + s)] = re[c]; A[2 * (c * n + s) + 1] = im[c]; }
+    }
+}
+// Pw[ky][kx] = 1/2 sum_c |sum_j A[c][j][kx] exp(-2 pi i ky j / ny)|^2 / (nx ny)^2, one thread per (ky, kx)
+ARK_GLOBAL void ark_k_spec_cols(ArkParams P, const double* __restrict__ A, const double* __restrict__ twy, double* __restrict__ Pw) {
+    const long long n = (long long)P.nx * P.ny;
+    const double norm = 1.0 / ((double)n * (double)n);
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const int kx = (int)(s % P.nx), ky = (int)(s / P.nx);
+        double pw = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            double re = 0.0, im = 0.0;
+            int t = 0;
+            for (int j = 0; j < P.ny; ++j) {
+                const double ar = A[2 * (c * n + (long long)j * P.nx + kx)], ai = A[2 * (c * n + (long long)j * P.nx + kx) + 1];
+                const double cs = twy[2 * t], sn = twy[2 * t + 1];
+                re += ar * cs + ai * sn;                   // (ar + i ai)(cs - i sn)
+                im += ai * cs - ar * sn;
+                t += ky; if (t >= P.ny) t -= P.ny;
+            }
+            pw += re * re + im * im;
+        }
+        Pw[s] = 0.5 * pw * norm;
+    }
+}
+// E[kappa] = sum of Pw over the shell of kappa: one block per kappa, fixed order
+ARK_GLOBAL void ark_k_spec_bins(ArkParams P, const double* __restrict__ Pw, double* __restrict__ E) {
+    ARK_SHARED double red[256];
+    const int kappa = blockIdx.x;
+    const long long n = (long long)P.nx * P.ny;
+    double acc = 0.0;
+    for (long long s = threadIdx.x; s < n; s += blockDim.x) {
+        int kx = (int)(s % P.nx), ky = (int)(s / P.nx);
+        if (2 * kx > P.nx) kx -= P.nx;
+        if (2 * ky > P.ny) ky -= P.ny;
+        const int b = (int)floor(sqrt((double)(kx * kx + ky * ky)) + 0.5);
+        if (b == kappa) acc += Pw[s];
+    }
+    red[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) E[kappa] = red[0];
+}
+#endif
+
+// ------------------------------------------------------------------------------------------------
 // fp64 pipe microbenchmark (measurement support for the "alu" roofline of bench.py): register-resident DFMA chains,
 // 8 independent chains per thread, no memory traffic.  One DFMA = one fp64 instruction (SURVEY 8(d) asks for a
 // MEASURED fp64 peak next to the measured HBM peak).

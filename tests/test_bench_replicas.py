@@ -126,7 +126,8 @@ def test_two_ranks_launched_by_torch_distributed_run(tmp_path):
     out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
                           "127.0.0.1", "--master-port", str(_free_port()), str(worker)], capture_output=True, text=True, timeout=300)
     assert out.returncode == 0, out.stderr[-2000:]
-    lines = [ln.split() for ln in out.stdout.splitlines() if ln.startswith("RANK")]
-    assert len(lines) == 2
+    import re
+    lines = re.findall(r"RANK (\d) (\S+) (\S+)", out.stdout)          # (the two ranks' lines may share one output line)
+    assert sorted(ln[0] for ln in lines) == ["0", "1"], out.stdout
     for ln in lines:
-        assert float(ln[2]) == 15.0 and abs(float(ln[3]) - 2 * 1000 * 4 / 15e-3) < 1e-6
+        assert float(ln[1]) == 15.0 and abs(float(ln[2]) - 2 * 1000 * 4 / 15e-3) < 1e-6

@@ -865,3 +865,38 @@ def test_array_potential_reduces_to_constant_gravity_and_keeps_the_two_energy_fo
     Uc = [col(rho), col(0 * rho), col(0 * rho), None, col(rho / 0.4)]
     S, _ = O.run(dict(prmc, phi=col(Phic)), Uc, 400, cfl=0.4)
     assert np.abs(S[2] / S[0]).max() < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# mid-plane kinetic-energy spectrum (reading A26)
+# ---------------------------------------------------------------------------------------------------------------
+def test_ke_spectrum_parseval_single_mode_and_brute_force():
+    rng = np.random.default_rng(5)
+    nx, ny, nz = 12, 10, 8
+    prm = I.make_params(nx, ny, nz, 0.1, 1.4)
+    rho = 0.5 + rng.random((nz, ny, nx))
+    vel = [rng.standard_normal((nz, ny, nx)) for _ in range(3)]
+    U = [rho, rho * vel[0], rho * vel[1], rho * vel[2], np.ones((nz, ny, nx))]
+    E = O.ke_spectrum(prm, U)
+    k = nz // 2
+    # Parseval: the shells add up to the plane mean of 1/2 rho |u|^2
+    mean_ke = float((0.5 * rho[k] * (vel[0][k] ** 2 + vel[1][k] ** 2 + vel[2][k] ** 2)).mean())
+    assert abs(E.sum() - mean_ke) < 1e-13 * mean_ke
+    assert E.size == int(np.floor(np.hypot(nx // 2, ny // 2) + 0.5)) + 1
+    # brute force: the double sum of the definition, term by term
+    j, i = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    brute = np.zeros(E.size)
+    for qy in range(ny):
+        for qx in range(nx):
+            ph = np.exp(-2j * np.pi * (qx * i / nx + qy * j / ny))
+            pw = sum(0.5 * abs((np.sqrt(rho[k]) * vel[c][k] * ph).sum() / (nx * ny)) ** 2 for c in range(3))
+            sx, sy = (qx if 2 * qx <= nx else qx - nx), (qy if 2 * qy <= ny else qy - ny)
+            brute[int(np.floor(np.hypot(sx, sy) + 0.5))] += pw
+    assert np.abs(E - brute).max() < 1e-13 * brute.max()
+    # one Fourier mode u = a cos(2 pi (3 i / nx + 2 j / ny)), rho = 1: |w^| = a/2 at +-(3,2), shell round(sqrt(13)) = 4, E = a^2/4
+    a = 0.7
+    u = a * np.cos(2 * np.pi * (3 * i / nx + 2 * j / ny))
+    one = np.ones((nz, ny, nx))
+    E1 = O.ke_spectrum(prm, [one, one * u[None], 0 * one, 0 * one, one])
+    expect = np.zeros(E.size); expect[4] = a * a / 4
+    assert np.abs(E1 - expect).max() < 1e-15

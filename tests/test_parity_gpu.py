@@ -743,3 +743,24 @@ def test_strict_build_shows_the_momentum_floor_is_rounding(B):
         r = res[name]
         assert r["abs"][0] <= 16 * 2.0 ** -52 * r["scale"][0] and r["abs"][4] <= 16 * 2.0 ** -52 * r["scale"][4], (name, r)
         assert max(r["abs"][1:4]) <= max(2 * r["floor"], 16 * 2.0 ** -52 * max(r["scale"][1:4])), (name, r)
+
+
+def test_ke_spectrum_matches_oracle(B):
+    """Mid-plane kinetic-energy power spectrum (reading A26) through ark_ke_spectrum, against the
+    oracle's FFT-based definition: random state on a ragged grid, the config-4 workload after 20 steps, and Parseval."""
+    for prm, U, nsteps in ((*I.random_state(45, 38, 12, 61), 0), (*I.config4_rb3d(64), 20)):
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        if nsteps:
+            s.run(nsteps, 0.4)
+        got = np.array(s.ke_spectrum())
+        state = to_np(s.get_state())
+        s.close()
+        ref = O.ke_spectrum(prm, state)
+        assert got.shape == ref.shape
+        assert np.abs(got - ref).max() <= 1e-12 * ref.max(), (prm["nx"], float(np.abs(got - ref).max()), float(ref.max()))
+        nx, ny, nz = prm["nx"], prm["ny"], prm["nz"]
+        S = [a.reshape(nz, ny, nx) for a in state]
+        k = nz // 2
+        mean_ke = float((0.5 * (S[1][k] ** 2 + S[2][k] ** 2 + S[3][k] ** 2) / S[0][k]).mean())
+        assert abs(got.sum() - mean_ke) <= 1e-12 * mean_ke
