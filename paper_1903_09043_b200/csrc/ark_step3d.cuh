@@ -69,8 +69,8 @@ struct ArkCfg3 {
     static constexpr int GB_OFF = YB_OFF + 5 * NS;                   // [4][NS]       dxv,dxu,dzv,dzw of row b (VISC)
     static constexpr int EB_OFF = GB_OFF + (VISC ? 4 : 0) * NS;      // [2][2][5][RX]  rho,v,p,rc,irc of the two edge rows, planes q, q+1
     static constexpr int RED_OFF = EB_OFF + 20 * RX;                 // [32] block reduction of the rate
-    static constexpr int MBAR_OFF = RED_OFF + 32;                    // [3] mbarriers of the UR slots
-    static constexpr int SMEM_DOUBLES = MBAR_OFF + 4;
+    static constexpr int MBAR_OFF = RED_OFF + 32;                    // [3] mbarriers of the UR slots, [3] TMEM base, [4] mbarrier of barrier B
+    static constexpr int SMEM_DOUBLES = MBAR_OFF + 6;
     static constexpr size_t SMEM_BYTES = (size_t)SMEM_DOUBLES * sizeof(double);
     static_assert((5 * NCOL * sizeof(double)) % 128 == 0, "TMA destination slots must stay 128-byte aligned");
     static_assert(((NWARP + 3) / 4) * 144 <= 512, "TMEM scratch columns of the warps that share a lane quarter");
@@ -87,6 +87,7 @@ struct ArkMarch3 {
     int tx, ty;                          // box origin in the padded array (columns, rows)
     unsigned long long* mbar;            // the block's three mbarriers (one per UR slot)
     unsigned phase;                      // parity bit of each slot's next completion
+    unsigned bphase;                     // parity of the next completion of barrier B (split arrive / wait)
     double* Ocur;                        // row a, plane q-1 of the output state (row b: + px)
     long long pstride, fs;
     int px;
@@ -136,6 +137,34 @@ ARK_DEV void ark_ring_wait3(ArkMarch3<VISC, TX, NW>& M, int slot) {
     M.phase ^= 1u << slot;
 #else
     (void)M; (void)slot;
+#endif
+}
+
+// Block barrier (B) of a plane as a SPLIT barrier: every warp arrives (one elected lane, after __syncwarp, on an
+// mbarrier that counts warps) as soon as its faces / differences / primitives are in shared memory, goes on with work
+// that only needs its own data, and waits right before it reads a neighbour's.  A warp that is ahead keeps issuing
+// instead of leaving its scheduler to a single, latency-bound warp.  ARK_SPLIT_B == 0: plain __syncthreads at the arrive.
+#ifndef ARK_SPLIT_B
+#define ARK_SPLIT_B 0
+#endif
+template <bool VISC, int TX, int NW>
+ARK_DEV void ark_bar_arrive(ArkMarch3<VISC, TX, NW>& M) {
+#if !defined(ARK_HOST_EMU) && ARK_SPLIT_B
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0)
+        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ark_smem_u32(M.mbar + 4)) : "memory");
+#else
+    (void)M;
+    __syncthreads();
+#endif
+}
+template <bool VISC, int TX, int NW>
+ARK_DEV void ark_bar_wait(ArkMarch3<VISC, TX, NW>& M) {
+#if !defined(ARK_HOST_EMU) && ARK_SPLIT_B
+    ark_mbar_wait(M.mbar + 4, M.bphase);
+    M.bphase ^= 1u;
+#else
+    (void)M;
 #endif
 }
 
@@ -473,18 +502,47 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     if (VISC && ROLE != 2) {                                      // row b's differences feed the low-y face of the pair above
         M.GB[s] = dxv[1]; M.GB[NT + s] = dxu[1]; M.GB[2 * NT + s] = dzv[1]; M.GB[3 * NT + s] = dzw[1];
     }
-    __syncthreads();                                              // (B) faces, differences (and prims q+1) visible
+    ark_bar_arrive(M);                                            // (B) faces, differences (and prims q+1) written
 
-    // ---------------- S3: acoustic update U~(q), PAPER.md:158-160 (+ reading A3 for the energy)
-    double Tp[2][5], acc[2][5], gpz[2][4];                        // parked z pipeline of the tile rows
+    // ---------------- between arrive and wait: what needs no neighbour -- the parked z pipeline of the tile rows and the
+    // dissipative fluxes (reading A6) through the x-, z- and (a|b) faces, in lock-step
+    double Tp[2][5], acc[2][5], gpz[2][4];
+    ArkVisc vyl = {0, 0, 0, 0}, vx[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}}, vz[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}}, vyi = {0, 0, 0, 0};
     if (ROLE == 1) {
 #pragma unroll
         for (int r = 0; r < 2; ++r) {
+            if (VISC) ark_tm_ld4(tm + ARK_TM_GZ(r), gpz[r][0], gpz[r][1], gpz[r][2], gpz[r][3]);
             ark_tm_get5(tm + ARK_TM_TP(r), Tp[r]);
             ark_tm_get5(tm + ARK_TM_AC(r), acc[r]);
-            if (VISC) ark_tm_ld4(tm + ARK_TM_GZ(r), gpz[r][0], gpz[r][1], gpz[r][2], gpz[r][3]);
+        }
+        ark_tm_wait_ld();
+        if (VISC) {
+            ArkViscIn in[5];
+            ArkVisc out[5];
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                const ArkPrim& c = wc[r];
+                // face (i-1 | i), normal x, transverse a = y, b = z
+                const ArkViscIn v1 = {c.u - Lu[r], c.v - Lv[r], c.w - Lw[r], ark_xl(dyu[r]) + dyu[r], ark_xl(dyv[r]) + dyv[r],
+                                      ark_xl(dzu[r]) + dzu[r], ark_xl(dzw[r]) + dzw[r], Lu[r] + c.u, Lv[r] + c.v, Lw[r] + c.w, c.T - LT[r]};
+                in[r] = v1;
+                // face (q-1 | q), normal z, transverse a = x, b = y
+                const double um = wm[r][0], vm = wm[r][1], wmm = wm[r][2], Tm = wm[r][3];
+                const ArkViscIn v2 = {c.w - wmm, c.u - um, c.v - vm, gpz[r][0] + dxw[r], gpz[r][1] + dxu[r], gpz[r][2] + dyw[r],
+                                      gpz[r][3] + dyv[r], wmm + c.w, um + c.u, vm + c.v, c.T - Tm};
+                in[2 + r] = v2;
+            }
+            const ArkPrim &a = wc[0], &b = wc[1];                 // face (a | b), normal y, transverse a = x, b = z
+            const ArkViscIn v3 = {b.v - a.v, b.u - a.u, b.w - a.w, dxv[0] + dxv[1], dxu[0] + dxu[1], dzv[0] + dzv[1],
+                                  dzw[0] + dzw[1], a.v + b.v, a.u + b.u, a.w + b.w, b.T - a.T};
+            in[4] = v3;
+            ark_visc_face_n<5>(P.D.KV, in, out);
+            vx[0] = out[0]; vx[1] = out[1]; vz[0] = out[2]; vz[1] = out[3]; vyi = out[4];
         }
     }
+    ark_bar_wait(M);                                              // (B) the neighbours' faces, differences visible
+
+    // ---------------- S3: acoustic update U~(q), PAPER.md:158-160 (+ reading A3 for the energy)
     ArkFace fyu = {0, 0, 0};                                      // high-y face of row b = low-y face of the pair above
     if (ROLE != 2) {
         fyu.us = M.FB[s + RX]; fyu.pi = M.FB[NT + s + RX];
@@ -543,42 +601,13 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         tb[0] = Ut[1][0]; tb[NT] = Ut[1][1]; tb[2 * NT] = Ut[1][2]; tb[3 * NT] = Ut[1][3]; tb[4 * NT] = Ut[1][4];
     }
 
-    // dissipative fluxes (reading A6) in lock-step: low-y face of row a; tile rows: x-, z- faces, (a|b)
-    ArkVisc vyl = {0, 0, 0, 0}, vx[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}}, vz[2] = {{0, 0, 0, 0}, {0, 0, 0, 0}}, vyi = {0, 0, 0, 0};
-    if (ROLE == 1) ark_tm_wait_ld();
+    // dissipative flux through the low-y face of row a (needs the differences of the pair below)
     if (VISC && ROLE != 0) {
-        constexpr int NV = ROLE == 1 ? 6 : 1;
-        ArkViscIn in[NV];
-        ArkVisc out[NV];
-        {
-            const double* g = M.GB + (s - RX);                   // dxv,dxu,dzv,dzw of row a-1
-            const ArkPrim& c = wc[0];
-            const ArkViscIn v = {c.v - Bm.v, c.u - Bm.u, c.w - Bm.w, g[0] + dxv[0], g[NT] + dxu[0], g[2 * NT] + dzv[0],
-                                 g[3 * NT] + dzw[0], Bm.v + c.v, Bm.u + c.u, Bm.w + c.w, c.T - Bm.T};
-            in[0] = v;
-        }
-        if (ROLE == 1) {
-#pragma unroll
-            for (int r = 0; r < 2; ++r) {
-                const ArkPrim& c = wc[r];
-                // face (i-1 | i), normal x, transverse a = y, b = z
-                const ArkViscIn v1 = {c.u - Lu[r], c.v - Lv[r], c.w - Lw[r], ark_xl(dyu[r]) + dyu[r], ark_xl(dyv[r]) + dyv[r],
-                                      ark_xl(dzu[r]) + dzu[r], ark_xl(dzw[r]) + dzw[r], Lu[r] + c.u, Lv[r] + c.v, Lw[r] + c.w, c.T - LT[r]};
-                in[1 + r] = v1;
-                // face (q-1 | q), normal z, transverse a = x, b = y
-                const double um = wm[r][0], vm = wm[r][1], wmm = wm[r][2], Tm = wm[r][3];
-                const ArkViscIn v2 = {c.w - wmm, c.u - um, c.v - vm, gpz[r][0] + dxw[r], gpz[r][1] + dxu[r], gpz[r][2] + dyw[r],
-                                      gpz[r][3] + dyv[r], wmm + c.w, um + c.u, vm + c.v, c.T - Tm};
-                in[3 + r] = v2;
-            }
-            const ArkPrim &a = wc[0], &b = wc[1];                 // face (a | b), normal y, transverse a = x, b = z
-            const ArkViscIn v3 = {b.v - a.v, b.u - a.u, b.w - a.w, dxv[0] + dxv[1], dxu[0] + dxu[1], dzv[0] + dzv[1],
-                                  dzw[0] + dzw[1], a.v + b.v, a.u + b.u, a.w + b.w, b.T - a.T};
-            in[NV - 1] = v3;
-        }
-        ark_visc_face_n<NV>(P.D.KV, in, out);
-        vyl = out[0];
-        if (ROLE == 1) { vx[0] = out[1]; vx[1] = out[2]; vz[0] = out[3]; vz[1] = out[4]; vyi = out[NV - 1]; }
+        const double* g = M.GB + (s - RX);                       // dxv,dxu,dzv,dzw of row a-1
+        const ArkPrim& c = wc[0];
+        const ArkViscIn v = {c.v - Bm.v, c.u - Bm.u, c.w - Bm.w, g[0] + dxv[0], g[NT] + dxu[0], g[2 * NT] + dzv[0],
+                             g[3 * NT] + dzw[0], Bm.v + c.v, Bm.u + c.u, Bm.w + c.w, c.T - Bm.T};
+        ark_visc_face_n<1>(P.D.KV, &v, &vyl);
     }
 
     if (ROLE == 1) {
@@ -817,7 +846,8 @@ ARK_DEV void ark_run_edge3(const ArkParams& P, ArkMarch3<VISC, TX, NW>& M, int e
         ark_edge_prims3(P, M, e, M.un, M.pn);         // plane q+1
         { const int t3 = M.uq; M.uq = M.un; M.un = M.unn; M.unn = t3; }
         { const int t2 = M.pc; M.pc = M.pn; M.pn = t2; }
-        __syncthreads();
+        ark_bar_arrive(M);
+        ark_bar_wait(M);
         __syncthreads();
     }
 }
@@ -902,11 +932,13 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     M.tx = (int)(blockIdx.x * TX) - 2 + ARK_XOFF;
     M.ty = (int)(blockIdx.y * TY) - 2 + ARK_NG;
     M.phase = 0;
+    M.bphase = 0;
     unsigned tmem_base = 0;
 #ifndef ARK_HOST_EMU
     unsigned* tm_slot = (unsigned*)(smem + C::MBAR_OFF + 3);
     if (t == 0) {
         for (int s3 = 0; s3 < 3; ++s3) ark_mbar_init(M.mbar + s3, 1);
+        ark_mbar_init(M.mbar + 4, C::NWARP);          // barrier B: one arrival per warp
         ark_mbar_fence_init();
     }
     if (t < 32) ark_tm_alloc_all(tm_slot);            // the whole TMEM of the SM (one block per SM)
