@@ -27,6 +27,7 @@
 #define ARK_K_IMPEDANCE 1.1  // a = K max(rho_L c_L, rho_R c_R), reading A2
 #define ARK_NG 2             // ghost layers (A9)
 #define ARK_XOFF 4           // x index of interior cell 0 inside a padded row (>= ARK_NG)
+#define ARK_MAX_ZCHUNKS 16   // z chunks of the 3D step kernel (blocks per column)
 
 enum { ARK_BCK_PERIODIC = 0, ARK_BCK_REFLECTING = 1, ARK_BCK_FIXED_T = 2, ARK_BCK_FLUX = 3, ARK_BCK_EXTERNAL = 4 };
 
@@ -56,6 +57,9 @@ struct ArkParams {
     // (PAPER.md:55, :152), padded like a state field with its ghost values already filled (reading A25); NULL = -g.x
     int eform;
     const double* phi;
+    // 3D step kernel: planes [zb[c], zb[c+1]) of z chunk c = blockIdx.z (chunk sizes decrease so that the last wave of
+    // blocks is short; chosen by a scheduling simulation in ark_create)
+    int zb[ARK_MAX_ZCHUNKS + 1];
 };
 
 inline void ark_fill_derived(ArkParams& P) {

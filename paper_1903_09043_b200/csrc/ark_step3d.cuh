@@ -886,8 +886,13 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     M.s = prow * RX + lane;
     M.ca = (2 * prow) * RX + lane;
     const int gi = blockIdx.x * TX - 2 + lane, gja = blockIdx.y * TY - 2 + 2 * prow;   // interior-based cell coordinates (row a)
-    M.k0 = blockIdx.z * zchunk;
-    M.k1 = M.k0 + zchunk < P.nz ? M.k0 + zchunk : P.nz;
+    if (zchunk > 0) {                                           // uniform chunks (tests); 0: the table of ark_create
+        M.k0 = blockIdx.z * zchunk;
+        M.k1 = M.k0 + zchunk < P.nz ? M.k0 + zchunk : P.nz;
+    } else {
+        M.k0 = P.zb[blockIdx.z];
+        M.k1 = P.zb[blockIdx.z + 1];
+    }
     const bool tile = pair >= 1 && pair <= NW - 2;
     const bool inx = lane >= 2 && lane < 2 + TX && gi < P.nx;
     M.inU[0] = tile && inx && gja < P.ny;
