@@ -305,13 +305,14 @@ namespace {
 
 // Time (in plane iterations) the grid of the 3D step kernel takes when its blocks are handed out in blockIdx order (x, y,
 // then z chunk) to nsm SMs, one block per SM, each block costing its planes + ~2.5 planes of prologue.
+double g_chunk_ovh = 2.5;                                     // prologue of a chunk in plane iterations (ARK_CHUNK_OVH overrides: tuning)
 double chunk_makespan(long long ncol, const int* chunk, int nchunk, int nsm) {
     std::vector<double> heap((size_t)nsm, 0.0);               // min-heap of the SMs' finish times
     auto cmp = [](double a, double b) { return a > b; };
     for (int c = 0; c < nchunk; ++c)
         for (long long b = 0; b < ncol; ++b) {
             std::pop_heap(heap.begin(), heap.end(), cmp);
-            heap.back() += chunk[c] + 2.5;
+            heap.back() += chunk[c] + g_chunk_ovh;
             std::push_heap(heap.begin(), heap.end(), cmp);
         }
     return *std::max_element(heap.begin(), heap.end());
@@ -323,6 +324,7 @@ double chunk_makespan(long long ncol, const int* chunk, int nchunk, int nsm) {
 // nchunk 1..16 x ratio 1 .. 0.4, scored by the scheduling simulation above.  zb[0..nchunk] = chunk boundaries.
 int choose_zchunks(int nx, int ny, int nz, int nsm, int* zb) {
     const long long ncol = (long long)((nx + TX3 - 1) / TX3) * ((ny + TY3 - 1) / TY3);
+    if (const char* e = getenv("ARK_CHUNK_OVH")) { const double v = atof(e); if (v > 0.0) g_chunk_ovh = v; }
     const double ratios[7] = {1.0, 0.9, 0.8, 0.7, 0.6, 0.5, 0.4};
     int best[ARK_MAX_ZCHUNKS] = {nz}, nbest = 1;
     double best_t = 1e300;
@@ -338,7 +340,7 @@ int choose_zchunks(int nx, int ny, int nz, int nsm, int* zb) {
             for (int i = 0; i < n; ++i) { ch[i] = (int)std::floor(nz * w / sum + 0.5); if (ch[i] < 4) ch[i] = 4; tot += ch[i]; w *= ratios[ir]; }
             ch[0] += nz - tot;
             if (ch[0] < 4 || (n > 1 && ch[0] < ch[1])) continue;
-            const double t = big ? (double)((ncol * n + nsm - 1) / nsm) * (nz / (double)n + 2.5) : chunk_makespan(ncol, ch, n, nsm);
+            const double t = big ? (double)((ncol * n + nsm - 1) / nsm) * (nz / (double)n + g_chunk_ovh) : chunk_makespan(ncol, ch, n, nsm);
             if (t < best_t) { best_t = t; nbest = n; for (int i = 0; i < n; ++i) best[i] = ch[i]; }
             if (n == 1 || big) break;
         }
