@@ -87,7 +87,7 @@ struct ark_solver {
     double* stage;
     cudaStream_t stream;
     int rate_slots;         // >0: scratch[0..rate_slots) holds the per-block rates of the CURRENT state
-    bool xghost_valid;      // 3D, periodic x: the step kernel already wrote the x ghost columns of the current state
+    bool xghost_valid;      // periodic x: the step kernel already wrote the x ghost columns of the current state
     bool xyghost_valid;     // the x and y ghost sweeps already ran on the current state (ark_get_halo)
     dim3 step_grid;
     int zchunk;
@@ -171,7 +171,7 @@ int launch_bc_xy(ark_solver* s, double* U) {
     const ArkParams& P = s->P;
     if (s->xyghost_valid) return ARK_OK;
     if (P.bc[0][0] == ARK_BCK_PERIODIC) {
-        // (3D: the fused step kernel writes the periodic x ghost columns of the state it produces; the sweep is only
+        // (the fused step kernels write the periodic x ghost columns of the state they produce; the sweep is only
         // needed for a state that came from outside)
         if (!s->xghost_valid) {
             const long long n = 2LL * P.ny * P.nz * P.nf;
@@ -261,7 +261,7 @@ int do_step(ark_solver* s, double dt, const double* dt_dev) {
     }
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
-    s->xghost_valid = s->P.ndim == 3 && s->P.bc[0][0] == ARK_BCK_PERIODIC;
+    s->xghost_valid = s->P.bc[0][0] == ARK_BCK_PERIODIC;
     s->xyghost_valid = false;
     s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
     return ARK_OK;

@@ -271,6 +271,12 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
         const double n4 = GEN ? Uc[4] - lam * dG[4] + lam * (eformB ? suS : work) : Uc[4] - lam * dG[4] + K.dt * work;
         if (inU) {
             Uout[colbase] = n0; Uout[colbase + fs] = n1; Uout[colbase + 2 * fs] = n2; Uout[colbase + 3 * fs] = n4;
+            // periodic x: the first / last two columns also fill the opposite ghost columns of the new state,
+            // so that the next step needs no x ghost-fill launch (as in the 3D kernel)
+            if (P.bc[0][0] == ARK_BCK_PERIODIC && (gi < ARK_NG || gi >= P.nx - ARK_NG)) {
+                const long long w = colbase + (gi < ARK_NG ? P.nx : -P.nx);
+                Uout[w] = n0; Uout[w + fs] = n1; Uout[w + 2 * fs] = n2; Uout[w + 3 * fs] = n4;
+            }
             if (rate_scratch) rate_max = ark_rate_epilogue(P, 2, n0, n1, n2, 0.0, n4, P.D.inv_h, P.D.dcoef);
         }
     }

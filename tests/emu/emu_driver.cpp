@@ -104,8 +104,8 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
     grid.z = P.ndim == 3 ? (nz + zchunk - 1) / zchunk : 1;
     const bool visc = mu > 0.0 || kappa > 0.0;
     for (int s = 0; s < nsteps; ++s) {
-        if (P.bc[0][0] == ARK_BCK_PERIODIC && P.ndim == 3 && s > 0) {
-            // mirrors launch_bc in csrc/ark.cu: the 3D step kernel wrote the periodic x ghost columns itself
+        if (P.bc[0][0] == ARK_BCK_PERIODIC && s > 0) {
+            // mirrors launch_bc in csrc/ark.cu: the step kernel wrote the periodic x ghost columns itself
         } else if (P.bc[0][0] == ARK_BCK_PERIODIC) {
             emu_dim3 gp; gp.x = (unsigned)((2LL * ny * nz * P.nf + 63) / 64);
             ark_emu_launch(gp, 64, 0, [&] { ark_k_bc_x_periodic(P, cur); });
