@@ -23,6 +23,7 @@ def nvcc_cmd(out, extra=()):
     # tile parameters can be overridden from the environment for tuning runs (ARK_NW3=10 ARK_LOW3=8 python -m ...build --force)
     defs = ["-D%s=%d" % (k, int(os.environ.get(k, v))) for k, v in TILES.items()]
     defs += ["-D" + d for d in os.environ.get("ARK_EXTRA_DEFS", "").split()]
+    defs += os.environ.get("ARK_EXTRA_FLAGS", "").split()          # e.g. "-Xptxas -O2" (tuning runs)
     return (["nvcc", "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
              "-Xcompiler", "-fPIC", "-shared", "-o", out] + defs + list(extra)
             + [os.path.join(CSRC, s) for s in SOURCES])
