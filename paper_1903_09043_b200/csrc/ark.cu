@@ -33,7 +33,7 @@ constexpr int TX3 = ARK_TX3, NW3 = ARK_NW3;   // 3D: outputs per row, row pairs 
 constexpr int TY3 = 2 * NW3 - 4;
 constexpr int TX2 = ARK_TX2, TY2 = ARK_TY2;   // 2D
 
-#define ARK_KERNEL_REV "r2.5"
+#define ARK_KERNEL_REV "r2.6"
 constexpr int CFL_BLOCK = 256;
 #define ARK_MAX_TIMED 4096
 constexpr int MAX_SCRATCH = 1 << 16;          // per-block rate slots

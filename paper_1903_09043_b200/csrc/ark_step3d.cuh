@@ -152,6 +152,9 @@ ARK_DEV void ark_ring_wait3(ArkMarch3<VISC, TX, NW>& M, int slot) {
 #ifndef ARK_UNROLL2
 #define ARK_UNROLL2 0
 #endif
+#ifndef ARK_RING_EARLY
+#define ARK_RING_EARLY 1
+#endif
 #ifndef ARK_SPLIT_B
 #define ARK_SPLIT_B 0
 #endif
@@ -358,6 +361,41 @@ ARK_DEV void ark_face_flux_n(double (*F)[5], const bool* left, const double* con
     }
 }
 
+// Ring warps, one plane EARLY.  A ring warp (one row, no lock-step partner, sharing its scheduler with two tile warps) is
+// the last to reach barrier B if it computes all its faces there; but the x-, (a|b) and low-y faces and the x differences
+// of plane p only need primitives of plane p, which exist one iteration before they are used.  So they are computed
+// between barriers B and C of the previous iteration, where the ring warp has little else to do and would wait for the
+// tile warps, and parked in its unused TMEM columns; before barrier B only the z face (which needs plane p+1) is left.
+// Same functions, same inputs: the results are bit-identical.  w: primitives of the ring row at plane p; pslot: PB / EB
+// slot of plane p.
+#define ARK_TM_EARLY 64u                                       // 11 doubles in the (unused) U~ columns of a ring warp
+template <bool VISC, bool GXY, int TX, int NW, int ROLE>
+ARK_DEV void ark_ring_early3(const ArkParams& P, ArkMarch3<VISC, TX, NW>& M, const ArkPrim& w, int pslot) {
+    using C = ArkCfg3<VISC, TX, NW>;
+    constexpr int RX = C::RX, NP = C::NP, NT = C::NS;
+    constexpr int NFE = ROLE == 0 ? 2 : 3;
+    const int s = M.s;
+    const double ghx = GXY ? P.D.gh[0] : 0.0, ghy = GXY ? P.D.gh[1] : 0.0;
+    const double* e = M.EB + (pslot * 2 + (ROLE == 0 ? 0 : 1)) * 5 * RX + (s % RX);     // the edge row next to the ring row
+    const double lr = ark_xl(w.rho), Lu = ark_xl(w.u), lp = ark_xl(w.p), lrc = ark_xl(w.rc), lirc = ark_xl(w.irc);
+    ArkFaceIn in[NFE];
+    ArkFace out[NFE];
+    in[0] = ark_face_in(ghx, lr, Lu, lp, lrc, lirc, w.rho, w.u, w.p, w.rc, w.irc);
+    if (ROLE == 0) in[1] = ark_face_in(ghy, e[0], e[RX], e[2 * RX], e[3 * RX], e[4 * RX], w.rho, w.v, w.p, w.rc, w.irc);   // (edge | ring)
+    else           in[1] = ark_face_in(ghy, w.rho, w.v, w.p, w.rc, w.irc, e[0], e[RX], e[2 * RX], e[3 * RX], e[4 * RX]);   // (ring | edge)
+    if (ROLE == 2) {
+        const double* n = M.PBb + pslot * NP * NT + (s - RX);                           // row a-1 (pair below)
+        in[NFE - 1] = ark_face_in(ghy, n[0], n[2 * NT], n[4 * NT], n[5 * NT], n[6 * NT], w.rho, w.v, w.p, w.rc, w.irc);
+    }
+    ark_face_n<NFE>(P.theta, in, out);
+    double dxu = 0.0, dxv = 0.0;
+    if (VISC) { dxu = ark_xr(w.u) - Lu; dxv = ark_xr(w.v) - ark_xl(w.v); }
+    const unsigned a = M.tm + ARK_TM_EARLY;
+    ark_tm_st4(a, out[0].us, out[0].pi, out[0].S, out[1].us);
+    ark_tm_st4(a + 8, out[1].pi, out[1].S, dxu, dxv);
+    if (ROLE == 2) { ark_tm_st2(a + 16, out[2].us, out[2].pi); ark_tm_st1(a + 20, out[2].S); }
+}
+
 // GXY: gravity may have x / y components (false: only g_z, the x and y source terms vanish at compile time)
 // PAR >= 0: the parity of the plane inside the two-fold unrolled steady loop, which makes the alternating slots (TMEM
 // primitive slot, PB slot) compile-time constants; -1: read them from M
@@ -375,6 +413,7 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     const bool gx = GXY && P.D.g_on[0], gy = GXY && P.D.g_on[1];
     const double ghx = GXY ? P.D.gh[0] : 0.0, ghy = GXY ? P.D.gh[1] : 0.0;
     const unsigned tm = M.tm;
+    constexpr bool EARLY = ARK_RING_EARLY && ROLE != 1 && !GEN;   // ring warps: see ark_ring_early3
     const int tcur = PAR >= 0 ? PAR : M.tcur;
     const int pc = PAR >= 0 ? PAR : M.pc, pn = pc ^ 1;
     // GEN: every face has its own -(Phi_R - Phi_L) in place of g_d h; the gravity work
@@ -406,6 +445,12 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
     ark_tm_wait_st();
 #pragma unroll
     for (int r = R0; r <= R1; ++r) ark_tm_get_prim(tm + ARK_TM_PR(tcur, r), wc[r]);
+    double er[11] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};           // ring warps: what ark_ring_early3 parked for this plane
+    if (EARLY) {
+        ark_tm_ld4(tm + ARK_TM_EARLY, er[0], er[1], er[2], er[3]);
+        ark_tm_ld4(tm + ARK_TM_EARLY + 8, er[4], er[5], er[6], er[7]);
+        if (ROLE == 2) { ark_tm_ld2(tm + ARK_TM_EARLY + 16, er[8], er[9]); ark_tm_ld1(tm + ARK_TM_EARLY + 20, er[10]); }
+    }
     if (VISC) {
 #pragma unroll
         for (int r = R0; r <= R1; ++r) ark_tm_ld4(tm + ARK_TM_PR(tcur ^ 1, r), wm[r][0], wm[r][1], wm[r][2], wm[r][3]);
@@ -448,13 +493,23 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
         Bm.rho = n[0]; Bm.u = n[NT]; Bm.v = n[2 * NT]; Bm.w = n[3 * NT]; Bm.p = n[4 * NT]; Bm.rc = n[5 * NT]; Bm.irc = n[6 * NT];
         if (VISC) Bm.T = n[7 * NT];
     }
-    if (ROLE != 1) {
+    if (ROLE != 1 && !EARLY) {
         // the edge row of a ring pair (row a of pair 0, row b of pair NW-1) only enters the (a|b) face
         constexpr int RE = ROLE == 0 ? 0 : 1;
         const double* e = M.EB + (pc * 2 + RE) * 5 * RX + (s % RX);
         wc[RE].rho = e[0]; wc[RE].v = e[RX]; wc[RE].p = e[2 * RX]; wc[RE].rc = e[3 * RX]; wc[RE].irc = e[4 * RX];
     }
-    {
+    if (EARLY) {
+        // x-, (a|b), low-y faces and x differences of this plane come from TMEM (computed one iteration ago); only the
+        // z face is computed here
+        constexpr int r = R0;
+        const ArkPrim& c = wc[r];
+        const ArkFaceIn zin = ark_face_in(P.D.gh[2], c.rho, c.w, c.p, c.rc, c.irc, wn[r].rho, wn[r].w, wn[r].p, wn[r].rc, wn[r].irc);
+        ark_face_n<1>(P.theta, &zin, &zhi[r]);
+        fx[r].us = er[0]; fx[r].pi = er[1]; fx[r].S = er[2];
+        fyi.us = er[3]; fyi.pi = er[4]; fyi.S = er[5];
+        if (ROLE == 2) { fyl.us = er[8]; fyl.pi = er[9]; fyl.S = er[10]; }
+    } else {
         // faces in lock-step: x- and z+ of the active rows, low-y of row a (not for the low ring pair), (a|b)
         constexpr int NF = 2 * NA + (ROLE != 0 ? 2 : 1);
         ArkFaceIn in[NF];
@@ -489,9 +544,12 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
 #pragma unroll
         for (int r = R0; r <= R1; ++r) {
             const ArkPrim& c = wc[r];
-            Lv[r] = ark_xl(c.v);
-            dxu[r] = ark_xr(c.u) - Lu[r];
-            dxv[r] = ark_xr(c.v) - Lv[r];
+            if (EARLY) { dxu[r] = er[6]; dxv[r] = er[7]; }
+            else {
+                Lv[r] = ark_xl(c.v);
+                dxu[r] = ark_xr(c.u) - Lu[r];
+                dxv[r] = ark_xr(c.v) - Lv[r];
+            }
             dzv[r] = wn[r].v - wm[r][1];
             dzw[r] = wn[r].w - wm[r][2];
             if (ROLE == 1) {
@@ -745,6 +803,8 @@ ARK_DEV void ark_plane3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VIS
             ark_tm_put5(tm + ARK_TM_AC(1), acc[1]);               // row b is complete but for its high-y / high-z faces
         }
     }
+    // ring warps: the faces of plane q+1 that need no plane q+2, while the tile warps are busy with plane q
+    if (EARLY) ark_ring_early3<VISC, GXY, TX, NW, ROLE>(P, M, wn[R0], pn);
     __syncthreads();                                              // (C) U~(q) of the pair below visible
 
     // ---------------- S4: low-y face of row a
@@ -838,6 +898,7 @@ ARK_DEV void ark_run_pair3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<
         p[0] = wc0[0].u; p[NS] = wc0[0].v; p[2 * NS] = wc0[0].w;
     }
     __syncthreads();                                  // primitives of plane k0-1 visible to the neighbours
+    if (ARK_RING_EARLY && ROLE != 1 && !GEN) ark_ring_early3<VISC, GXY, TX, NW, ROLE>(P, M, wc0[ROLE == 0 ? 1 : 0], M.pc);   // plane k0-1
     ark_march3<VISC, GXY, GEN, TX, NW, ROLE>(P, K, M);
     ark_tm_wait_st();
 }

@@ -68,6 +68,8 @@ inline void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) {
 inline void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
     double* p = ark_emu_tm(a); p[0] = v0; p[1] = v1; p[2] = v2; p[3] = v3; p[4] = v4; p[5] = v5; p[6] = v6; p[7] = v7;
 }
+inline void ark_tm_st2(unsigned a, double v0, double v1) { double* p = ark_emu_tm(a); p[0] = v0; p[1] = v1; }
+inline void ark_tm_ld2(unsigned a, double& v0, double& v1) { const double* p = ark_emu_tm(a); v0 = p[0]; v1 = p[1]; }
 inline void ark_tm_ld1(unsigned a, double& v0) { v0 = ark_emu_tm(a)[0]; }
 inline void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) { const double* p = ark_emu_tm(a); v0 = p[0]; v1 = p[1]; v2 = p[2]; v3 = p[3]; }
 inline void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
