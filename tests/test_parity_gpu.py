@@ -732,7 +732,8 @@ def test_strict_build_shows_the_momentum_floor_is_rounding(B):
     from paper_1903_09043_b200 import build as cuda_build
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     lib = cuda_build.LIB_STRICT
-    assert os.path.exists(lib), "build the strict twin first: python -m paper_1903_09043_b200.build --strict (or __graft_entry__.build())"
+    if not os.path.exists(lib):
+        lib = cuda_build.build_strict()              # normally built by __graft_entry__.build(); nvcc is on the GPU box too
     env = dict(os.environ, ARK_B200_LIBRARY=lib)
     r = subprocess.run([sys.executable, "-c", _STRICT_SCRIPT % root], env=env, capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stderr[-2000:]
