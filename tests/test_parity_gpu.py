@@ -546,6 +546,9 @@ GENERAL = {
     "3d_phi_periodic_inviscid": lambda: (I.random_state(45, 21, 19, 45), 0, "periodic"),
     "3d_phi_walls_viscous": lambda: (I.random_state(41, 23, 30, 46, mu=1e-3, kappa=2e-3,
                                                     bc_type=((PER, PER), (REF, REF), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))), 0, "walls"),
+    # many z chunks of decreasing size (few columns, 70 planes) on the general path
+    "3d_phi_walls_appendix_b_many_chunks": lambda: (I.random_state(61, 37, 70, 48, mu=1e-3, kappa=2e-3,
+                                                                   bc_type=((PER, PER), (REF, REF), (FIX, REF)), bc_value=((0, 0), (0, 0), (2.5, 0))), 1, "walls"),
     "3d_phi_all_walls_appendix_b": lambda: (I.random_state(33, 20, 18, 47, mu=1e-3, kappa=0.0,
                                                            bc_type=((REF, REF), (REF, FIX), (REF, REF)), bc_value=((0, 0), (0, 3.5), (0, 0))), 1, "walls"),
 }
