@@ -89,6 +89,7 @@ struct ark_solver {
     int rate_slots;         // >0: scratch[0..rate_slots) holds the per-block rates of the CURRENT state
     bool xghost_valid;      // periodic x: the step kernel already wrote the x ghost columns of the current state
     bool xyghost_valid;     // the x and y ghost sweeps already ran on the current state (ark_get_halo)
+    bool yghost_valid;      // 2D, periodic x and y: the step kernel already wrote the y ghost rows (and corners) as well
     dim3 step_grid;
     int zchunk;
     long long launches;
@@ -183,7 +184,7 @@ int launch_bc_xy(ark_solver* s, double* U) {
         ark_k_bc<0><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
         s->launches++;
     }
-    {
+    if (!s->yghost_valid) {
         const long long n = 2LL * (P.nx + 2 * ARK_NG) * P.nz;
         ark_k_bc<1><<<grid_for(n, 128), 128, 0, s->stream>>>(P, U);
         s->launches++;
@@ -262,6 +263,7 @@ int do_step(ark_solver* s, double dt, const double* dt_dev) {
     if (rc != ARK_OK) return rc;
     s->cur = 1 - s->cur;
     s->xghost_valid = s->P.bc[0][0] == ARK_BCK_PERIODIC;
+    s->yghost_valid = s->P.ndim == 2 && s->xghost_valid && s->P.bc[1][0] == ARK_BCK_PERIODIC;
     s->xyghost_valid = false;
     s->rate_slots = (int)(s->step_grid.x * s->step_grid.y * s->step_grid.z);   // fused CFL epilogue filled them
     return ARK_OK;
@@ -537,6 +539,7 @@ int ark_set_state(ark_solver* s, const double* rho, const double* rhou, const do
     ARK_CUDA(cudaGetLastError());
     s->rate_slots = 0;
     s->xghost_valid = false;
+    s->yghost_valid = false;
     s->xyghost_valid = false;
     return ARK_OK;
 }
@@ -570,6 +573,7 @@ int ark_set_state_host(ark_solver* s, const double* rho, const double* rhou, con
     ARK_CUDA(cudaStreamSynchronize(s->stream));
     s->rate_slots = 0;
     s->xghost_valid = false;
+    s->yghost_valid = false;
     s->xyghost_valid = false;
     return ARK_OK;
 }

@@ -273,9 +273,15 @@ ARK_DEV void ark_step2d(const ArkParams& P, const double* __restrict__ Uin, doub
             Uout[colbase] = n0; Uout[colbase + fs] = n1; Uout[colbase + 2 * fs] = n2; Uout[colbase + 3 * fs] = n4;
             // periodic x: the first / last two columns also fill the opposite ghost columns of the new state,
             // so that the next step needs no x ghost-fill launch (as in the 3D kernel)
-            if (P.bc[0][0] == ARK_BCK_PERIODIC && (gi < ARK_NG || gi >= P.nx - ARK_NG)) {
-                const long long w = colbase + (gi < ARK_NG ? P.nx : -P.nx);
-                Uout[w] = n0; Uout[w + fs] = n1; Uout[w + 2 * fs] = n2; Uout[w + 3 * fs] = n4;
+            const bool perx = P.bc[0][0] == ARK_BCK_PERIODIC, pery = perx && P.bc[1][0] == ARK_BCK_PERIODIC;
+            const long long wx = (perx && gi < ARK_NG) ? P.nx : ((perx && gi >= P.nx - ARK_NG) ? -P.nx : 0);
+            // (the y ghost rows are only written here when x is periodic too: their corner cells then come from this kernel
+            // as well; with walls in x the y sweep of the ghost-fill kernel copies the wall ghosts of the wrapped rows)
+            if (wx != 0) { const long long w = colbase + wx; Uout[w] = n0; Uout[w + fs] = n1; Uout[w + 2 * fs] = n2; Uout[w + 3 * fs] = n4; }
+            if (pery && (gj < ARK_NG || gj >= P.ny - ARK_NG)) {      // (uniform test first: nothing of this for wall configurations)
+                const long long wy = gj < ARK_NG ? (long long)P.px * P.ny : -(long long)P.px * P.ny;
+                { const long long w = colbase + wy; Uout[w] = n0; Uout[w + fs] = n1; Uout[w + 2 * fs] = n2; Uout[w + 3 * fs] = n4; }
+                if (wx != 0) { const long long w = colbase + wx + wy; Uout[w] = n0; Uout[w + fs] = n1; Uout[w + 2 * fs] = n2; Uout[w + 3 * fs] = n4; }
             }
             if (rate_scratch) rate_max = ark_rate_epilogue(P, 2, n0, n1, n2, 0.0, n4, P.D.inv_h, P.D.dcoef);
         }

@@ -112,7 +112,8 @@ int emu_run(int nx, int ny, int nz, double h, double gamma, const double* g, dou
         } else {
             bc<0>(P, cur, 2LL * ny * nz);
         }
-        bc<1>(P, cur, 2LL * (nx + 4) * nz);
+        if (!(P.ndim == 2 && s > 0 && P.bc[0][0] == ARK_BCK_PERIODIC && P.bc[1][0] == ARK_BCK_PERIODIC))   // (2D, fully periodic: the step kernel wrote them)
+            bc<1>(P, cur, 2LL * (nx + 4) * nz);
         if (P.ndim == 3) bc<2>(P, cur, 2LL * (nx + 4) * (ny + 4));
         if (s == 0 && padded_out) {
             const int mx = nx + 4;
