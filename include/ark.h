@@ -86,6 +86,41 @@ int ark_get_state_host(ark_solver*, double* rho, double* rhou, double* rhov, dou
  * Returns ARK_ENONFINITE if the maximum rate is not finite and positive. */
 int ark_compute_dt(ark_solver*, double cfl, double* dt_out);
 
+/* The same CFL time step for callers that cannot allocate device memory: no handle, no workspace, no cudaMalloc /
+ * cudaFree / cudaMallocHost and no allocating library routine anywhere on this path.
+ *
+ * Who that is: every other entry point needs an ark_solver, and a solver needs a workspace of ark_workspace_bytes() that
+ * somebody must allocate (two padded copies of the state).  A code that only wants to ask "what time step would ARK take
+ * on this state?" -- a coupling or in-situ analysis plug-in running inside a host application whose own memory pool has
+ * already claimed the GPU, or a time loop that must not pay the device-wide synchronisation cudaMalloc and cudaFree imply
+ * -- has the five dense fields on the device and nowhere to put a workspace.  Here the only scratch the reduction needs
+ * (one double per block of its first pass) lives inside the library image: a static 256 KiB device array that each GPU
+ * which loads the library holds until the process exits.
+ *
+ * rho .. E: DEVICE, dense interior-only fields as everywhere in this header (nx*ny*nz doubles, x fastest; rhow may be NULL
+ * when nz == 1), read in place, never copied.  d_out: DEVICE, 2 doubles, written as { max rate, cfl / max rate } with the
+ * rate of ark_compute_dt (reading A4).  Asynchronous on cuda_stream; nothing is synchronised and nothing is checked on
+ * the host, so a state without a finite positive maximum rate shows as a NaN / non-positive d_out[0] (NaN-propagating
+ * max), not as ARK_ENONFINITE.
+ *
+ * Limit: nx*ny*nz <= ark_cfl_dt_static_max_cells() = 2^27 = 134 217 728 cells (512^3: 32 768 scratch slots x 4096 cells
+ * per block).  Larger grids are rejected with ARK_EINVAL before anything is launched; use ark_compute_dt for them.
+ *
+ * First call on a device: the library looks up the device address of its scratch array for the device that is current
+ * (once per device, cached).  Make that first call outside any stream capture; later calls only launch two kernels.
+ *
+ * Sharing: there is ONE scratch array per GPU, shared by every call from every thread and stream, and it keeps whatever
+ * the previous call left in it.  Nothing in it has to start at zero -- each call overwrites the slots it is going to
+ * read before reading them, so a smaller grid after a larger one is safe -- but two calls that are in flight on the same
+ * GPU at the same time (different streams, or different host threads on streams that are not ordered with each other)
+ * race on the array and may both return garbage.  Order them (same stream, or events).
+ * Errors: ARK_EINVAL (sizes as for ark_create, too many cells, dx/gamma/mu/kappa/cfl out of range, NULL pointer),
+ * ARK_ECUDA. */
+size_t ark_cfl_dt_static_max_cells(void);
+int ark_cfl_dt_static(int nx, int ny, int nz, double dx, double gamma, double mu, double kappa,
+                      const double* rho, const double* rhou, const double* rhov, const double* rhow, const double* E,
+                      double cfl, double* d_out, void* cuda_stream);
+
 /* Advance the state by one full step of size dt (ghost fill, acoustic + transport + dissipative
  * fluxes, conservative update).  Asynchronous on the stream. */
 int ark_step(ark_solver*, double dt);

@@ -18,7 +18,7 @@ ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
 BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
-           "ark_get_state_host", "ark_compute_dt", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
+           "ark_get_state_host", "ark_compute_dt", "ark_cfl_dt_static", "ark_cfl_dt_static_max_cells", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
            "ark_halo_bytes", "ark_get_halo", "ark_set_halo", "ark_ke_spectrum_bins", "ark_ke_spectrum",
            "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
@@ -57,6 +57,10 @@ def load():
         getattr(lib, name).restype = ip
     lib.ark_compute_dt.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
     lib.ark_compute_dt.restype = ip
+    lib.ark_cfl_dt_static_max_cells.argtypes = []
+    lib.ark_cfl_dt_static_max_cells.restype = C.c_size_t
+    lib.ark_cfl_dt_static.argtypes = [ip, ip, ip, C.c_double, C.c_double, C.c_double, C.c_double] + [dp] * 5 + [C.c_double, dp, vp]
+    lib.ark_cfl_dt_static.restype = ip
     lib.ark_step.argtypes = [vp, C.c_double]
     lib.ark_step.restype = ip
     lib.ark_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
@@ -113,6 +117,40 @@ def workspace_bytes(nx, ny, nz):
 def _check(rc):
     if rc != ARK_OK:
         raise ArkError(rc, load().ark_last_error().decode())
+
+
+def cfl_dt_static_max_cells():
+    return int(load().ark_cfl_dt_static_max_cells())
+
+
+def cfl_dt_static(params, U, cfl, out, stream=None):
+    """ark_cfl_dt_static: the CFL time step of a dense device state without a Solver, a workspace or any allocation.
+
+    For callers that have the five fields on the GPU but may not allocate there (a plug-in inside an application whose
+    memory pool owns the device, a loop that must avoid the synchronisation of cudaMalloc / cudaFree): the reduction's
+    scratch is a fixed array inside the library, so grids are limited to cfl_dt_static_max_cells() = 2^27 cells.
+    U: [rho, rhou, rhov, rhow or None (2D), E], contiguous float64 CUDA tensors of nx*ny*nz elements, read in place.
+    out: float64 CUDA tensor of 2 elements supplied by the caller; receives [max rate, cfl / max rate].  Asynchronous on
+    `stream` (default: torch's current stream); calls that overlap on one GPU race on the shared scratch."""
+    lib = load()
+    nx, ny, nz = int(params["nx"]), int(params["ny"]), int(params["nz"])
+    ptrs = []
+    for f, a in enumerate(U):
+        if a is None:
+            if not (f == 3 and nz == 1):
+                raise ValueError("state field %d is None" % f)
+            ptrs.append(None)
+            continue
+        if a.dtype != torch.float64 or not a.is_contiguous() or a.numel() != nx * ny * nz or a.device.type != "cuda":
+            raise ValueError("state field %d must be a contiguous float64 CUDA tensor of %d elements" % (f, nx * ny * nz))
+        ptrs.append(C.c_void_p(a.data_ptr()))
+    if out.dtype != torch.float64 or not out.is_contiguous() or out.numel() != 2 or out.device.type != "cuda":
+        raise ValueError("out must be a contiguous float64 CUDA tensor of 2 elements")
+    st = stream if stream is not None else torch.cuda.current_stream(out.device)
+    _check(lib.ark_cfl_dt_static(nx, ny, nz, float(params["dx"]), float(params["gamma"]), float(params["mu"]),
+                                 float(params["kappa"]), *ptrs, float(cfl), C.c_void_p(out.data_ptr()),
+                                 C.c_void_p(st.cuda_stream)))
+    return out
 
 
 class Solver:

@@ -878,3 +878,108 @@ int ark_debug_get_padded(ark_solver* s, double* rho, double* rhou, double* rhov,
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// ark_cfl_dt_static: the CFL time step without any device allocation (see include/ark.h for who needs that and why).
+//
+// The two-pass max reduction needs one double of scratch per block of pass 1.  Every other entry point takes that
+// scratch from the caller's workspace; this one keeps it in the library image: a file-scope device array of
+// ARK_STATIC_SLOTS doubles (256 KiB) that every GPU which loads the library holds until the process exits.  Pass 1 is a
+// variant of ark_k_cfl_pass1 that reads the caller's DENSE fields directly (no padded copy, so no second buffer either)
+// and gives every block a fixed range of ARK_STATIC_BLOCK_CELLS cells, which is what bounds the grid size: at most
+// ARK_STATIC_SLOTS * ARK_STATIC_BLOCK_CELLS = 2^27 cells (512^3).
+//
+// In host code `g_static_rates` is only the host-side shadow of the symbol, not a device address; the address the kernels
+// get comes from cudaGetSymbolAddress, asked for once per device while that device is current (static_rates_ptr below).
+// ------------------------------------------------------------------------------------------------
+#define ARK_STATIC_SLOTS 32768
+#define ARK_STATIC_BLOCK_THREADS 256
+#define ARK_STATIC_CELLS_PER_THREAD 16
+#define ARK_STATIC_BLOCK_CELLS (ARK_STATIC_BLOCK_THREADS * ARK_STATIC_CELLS_PER_THREAD)
+#define ARK_STATIC_MAX_DEVICES 64
+
+static __device__ __align__(256) double g_static_rates[ARK_STATIC_SLOTS];
+
+// pass 1 on dense fields: block b owns cells [b * BLOCK_CELLS, (b + 1) * BLOCK_CELLS), coalesced strides of one block
+// width; slots[b] = NaN-propagating max of the cells' CFL rates.  Every slot a call reads is written by that call first.
+static __global__ void __launch_bounds__(ARK_STATIC_BLOCK_THREADS)
+ark_k_cfl_dense_pass1(ArkParams P, long long n, const double* __restrict__ rho, const double* __restrict__ mx,
+                      const double* __restrict__ my, const double* __restrict__ mz, const double* __restrict__ E,
+                      double* __restrict__ slots) {
+    __shared__ double red[32];
+    const double inv_h = 1.0 / P.h;
+    const double dcoef = 2.0 * P.ndim * fmax(4.0 * P.mu / 3.0, P.gm1 * P.kappa) * inv_h * inv_h;
+    const long long base = (long long)blockIdx.x * ARK_STATIC_BLOCK_CELLS + threadIdx.x;
+    double m = -1.0;
+#pragma unroll 4
+    for (int j = 0; j < ARK_STATIC_CELLS_PER_THREAD; ++j) {
+        const long long c = base + (long long)j * ARK_STATIC_BLOCK_THREADS;
+        if (c < n) m = ark_nanmax(m, ark_rate(P, rho[c], mx[c], my[c], P.ndim == 3 ? mz[c] : 0.0, E[c], inv_h, dcoef));
+    }
+    m = ark_block_nanmax(m, red);
+    if (threadIdx.x == 0) slots[blockIdx.x] = m;
+}
+
+// pass 2: one block over the nvals slots of this call; out[0] = max rate, out[1] = cfl / max rate
+static __global__ void ark_k_cfl_static_pass2(const double* __restrict__ slots, int nvals, double cfl, double* __restrict__ out) {
+    __shared__ double red[32];
+    double m = -1.0;
+    for (int s = threadIdx.x; s < nvals; s += blockDim.x) m = ark_nanmax(m, slots[s]);
+    m = ark_block_nanmax(m, red);
+    if (threadIdx.x == 0) { out[0] = m; out[1] = cfl / m; }
+}
+
+namespace {
+
+// Device address of g_static_rates on the CURRENT device, looked up once per device ordinal.  (The runtime resolves the
+// symbol against the current device's copy of the module, so the look-up must happen with that device current; the
+// result is a plain device pointer that stays valid until the process exits.)
+int static_rates_ptr(double** out) {
+    static double* cached[ARK_STATIC_MAX_DEVICES];     // zero-initialised; written once per device
+    int dev = -1;
+    ARK_CUDA(cudaGetDevice(&dev));
+    const bool slot = dev >= 0 && dev < ARK_STATIC_MAX_DEVICES;
+    double* p = slot ? __atomic_load_n(&cached[dev], __ATOMIC_ACQUIRE) : nullptr;
+    if (!p) {
+        void* q = nullptr;
+        ARK_CUDA(cudaGetSymbolAddress(&q, g_static_rates));
+        if (!q) return fail(ARK_ECUDA, "ark_cfl_dt_static: cudaGetSymbolAddress returned no address%s");
+        p = (double*)q;
+        if (slot) __atomic_store_n(&cached[dev], p, __ATOMIC_RELEASE);   // two racing threads store the same value
+    }
+    *out = p;
+    return ARK_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ark_cfl_dt_static_max_cells(void) { return (size_t)ARK_STATIC_SLOTS * ARK_STATIC_BLOCK_CELLS; }
+
+int ark_cfl_dt_static(int nx, int ny, int nz, double dx, double gamma, double mu, double kappa, const double* rho,
+                      const double* rhou, const double* rhov, const double* rhow, const double* E, double cfl,
+                      double* d_out, void* cuda_stream) {
+    if (!valid_sizes(nx, ny, nz)) return fail(ARK_EINVAL, "ark_cfl_dt_static: need nx,ny >= 4 and nz == 1 or nz >= 4, each <= 16384%s");
+    if (!(dx > 0.0) || !(gamma > 1.0) || !(mu >= 0.0) || !(kappa >= 0.0) || !(cfl > 0.0))
+        return fail(ARK_EINVAL, "ark_cfl_dt_static: need dx > 0, gamma > 1, mu,kappa >= 0, cfl > 0%s");
+    if (!rho || !rhou || !rhov || !E || (nz > 1 && !rhow) || !d_out) return fail(ARK_EINVAL, "ark_cfl_dt_static: NULL argument%s");
+    const long long n = (long long)nx * ny * nz;
+    if (n > (long long)ark_cfl_dt_static_max_cells())
+        return fail(ARK_EINVAL, "ark_cfl_dt_static: the grid has more cells than the library's built-in scratch serves%s (at most %lld = 512^3; "
+                                "larger grids: ark_compute_dt with a caller-allocated workspace)", "", (long long)ark_cfl_dt_static_max_cells());
+    double* slots = nullptr;
+    { const int rc = static_rates_ptr(&slots); if (rc != ARK_OK) return rc; }
+    ArkParams P;
+    memset(&P, 0, sizeof P);
+    P.nx = nx; P.ny = ny; P.nz = nz; P.ndim = nz > 1 ? 3 : 2;
+    P.h = dx; P.gamma = gamma; P.gm1 = gamma - 1.0; P.mu = mu; P.kappa = kappa;
+    const int nblocks = (int)((n + ARK_STATIC_BLOCK_CELLS - 1) / ARK_STATIC_BLOCK_CELLS);
+    const cudaStream_t st = (cudaStream_t)cuda_stream;
+    ark_k_cfl_dense_pass1<<<nblocks, ARK_STATIC_BLOCK_THREADS, 0, st>>>(P, n, rho, rhou, rhov, rhow, E, slots);
+    ark_k_cfl_static_pass2<<<1, 1024, 0, st>>>(slots, nblocks, cfl, d_out);
+    ARK_CUDA(cudaGetLastError());
+    return ARK_OK;
+}
+
+}  // extern "C"
