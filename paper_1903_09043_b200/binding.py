@@ -192,6 +192,9 @@ class Solver:
         self._h = h
         self._lib = lib
         self._phi_buf = None
+        # size queries are answered once here: get_halo / set_halo run every step of a slab run
+        self._halo_doubles = int(lib.ark_halo_bytes(self.nx, self.ny, self.nz)) // 8
+        self._potential_bytes = int(lib.ark_potential_bytes(self.nx, self.ny, self.nz))
         if int(params.get("energy_form", 0)) != 0:
             self.set_energy_form(int(params["energy_form"]))
         if params.get("phi") is not None:
@@ -209,7 +212,7 @@ class Solver:
             return
         if phi.dtype != torch.float64 or not phi.is_contiguous() or phi.numel() != self.n or phi.device.type != "cuda":
             raise ValueError("phi must be a contiguous float64 CUDA tensor of %d elements" % self.n)
-        nbytes = int(self._lib.ark_potential_bytes(self.nx, self.ny, self.nz))
+        nbytes = self._potential_bytes
         buf = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (buf.data_ptr() + 255) // 256 * 256
         _check(self._lib.ark_set_potential(self._h, C.c_void_p(phi.data_ptr()), C.c_void_p(ptr), C.c_size_t(nbytes)))
@@ -259,7 +262,7 @@ class Solver:
 
     # ------------------------------------------------------------------ slab decomposition (ARK_BC_EXTERNAL sides)
     def halo_doubles(self):
-        return int(self._lib.ark_halo_bytes(self.nx, self.ny, self.nz)) // 8
+        return self._halo_doubles
 
     def get_halo(self, side, out=None):
         """the two interior planes next to z side `side` (0 low, 1 high) with their x / y ghost cells -> CUDA tensor."""

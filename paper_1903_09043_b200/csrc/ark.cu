@@ -385,8 +385,14 @@ long long step_blocks(int nx, int ny, int nz, dim3* grid, int* zb, int nsm = 148
     return (long long)gx * gy;
 }
 
+// Cheap (the size queries ark_workspace_bytes / ark_potential_bytes / ark_halo_bytes go through it; the scheduling
+// simulation of choose_zchunks costs milliseconds and runs in ark_create only): choose_zchunks never takes more chunks
+// than the rate scratch has slots for and a single chunk is always allowed, so the grid fits exactly when its columns do.
 bool supported_grid(int nx, int ny, int nz) {
-    return valid_sizes(nx, ny, nz) && step_blocks(nx, ny, nz, nullptr, nullptr) <= MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG;
+    if (!valid_sizes(nx, ny, nz)) return false;
+    const long long ncol = nz > 1 ? (long long)((nx + TX3 - 1) / TX3) * ((ny + TY3 - 1) / TY3)
+                                  : (long long)((nx + TX2 - 1) / TX2) * ((ny + TY2 - 1) / TY2);
+    return ncol <= MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG;
 }
 
 }  // namespace

@@ -41,6 +41,23 @@ def test_version_and_workspace(lib):
     assert 10e9 < binding.workspace_bytes(512, 512, 512) < 14e9
 
 
+def test_size_queries_are_cheap_and_keep_the_documented_limits(lib):
+    """ark_workspace_bytes / ark_potential_bytes / ark_halo_bytes are called per step by a slab run (binding caches them
+    too): they must not run the z-chunk scheduling simulation of ark_create (milliseconds for 512^3)."""
+    import time
+    from paper_1903_09043_b200 import binding
+    assert binding.workspace_bytes(4096, 4096, 1) == 0                 # more fused-step blocks than rate slots (ark.h)
+    assert binding.workspace_bytes(2048, 2048, 1) > 0
+    assert binding.workspace_bytes(1024, 1024, 1024) > 0
+    assert lib.ark_halo_bytes(512, 512, 1) == 0 and lib.ark_potential_bytes(8, 8, 2) == 0
+    assert lib.ark_halo_bytes(512, 512, 64) == 5 * 2 * 528 * 516 * 8   # 5 fields x 2 padded planes (pitch 528)
+    t0 = time.perf_counter()
+    for _ in range(200):
+        lib.ark_halo_bytes(512, 512, 512)
+        lib.ark_workspace_bytes(512, 512, 128)
+    assert time.perf_counter() - t0 < 0.1                              # was 2 x 200 x ~10 ms
+
+
 def test_create_rejects_bad_arguments_without_touching_the_gpu(lib):
     from paper_1903_09043_b200 import binding
     h = C.c_void_p()
