@@ -82,7 +82,7 @@ int ark_get_state_host(ark_solver*, double* rho, double* rhou, double* rhov, dou
 
 /* CFL time step ("time step kernel"; formula = A4):
  *   dt = cfl / max_c [ sum_d (|u_d| + c)/dx + 2 ndim max(4 mu/3, (gamma-1) kappa) / (rho dx^2) ].
- * Deterministic two-pass max reduction (NaN-propagating).  Synchronises the stream (8-byte D2H).
+ * Deterministic two-pass max reduction (NaN-propagating).  Synchronises the stream (16-byte D2H).
  * Returns ARK_ENONFINITE if the maximum rate is not finite and positive. */
 int ark_compute_dt(ark_solver*, double cfl, double* dt_out);
 
@@ -160,8 +160,10 @@ int ark_set_potential(ark_solver*, const double* d_phi, void* d_buffer, size_t b
  * sub-domain hands out the two interior planes next to such a side (ark_get_halo) and receives the neighbour's into its
  * ghost planes (ark_set_halo); the time step is the minimum of the sub-domains' ark_compute_dt.  A halo is
  * ark_halo_bytes() bytes of DEVICE memory: [field][2 planes][ny+4 rows][row pitch], i.e. padded planes WITH their x / y
- * ghost cells (ark_get_halo runs the x and y ghost sweeps first; the following ark_step does not repeat them), so that the
- * assembled result is bit-identical to the undivided domain.  side: 0 = low z, 1 = high z.  Both calls are asynchronous
+ * ghost cells (ark_get_halo runs the x and y ghost sweeps first; the following ark_step does not repeat them), so that every
+ * cell sees the same neighbourhood as on the undivided domain: the assembled result is bit-identical to it in the strict
+ * build (-DARK_STRICT --fmad=false) and within a few ulp (1e-14 relative) in the product build, whose steady-state and
+ * boundary-plane code paths contract FMAs differently.  side: 0 = low z, 1 = high z.  Both calls are asynchronous
  * on the stream; the caller moves the buffers between devices (NCCL send/recv or peer copies over NVLink).  ark_run and
  * array-valued potentials are not available on sub-domains.  Errors: ARK_EINVAL (2D solver, bad side, side not
  * external), ARK_ECUDA. */

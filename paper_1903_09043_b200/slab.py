@@ -8,7 +8,13 @@ that face a neighbour are ARK_BC_EXTERNAL, and before every step
   2. exchanges them with its neighbours (torch.distributed P2P: NCCL over NVLink / NVSwitch on a B200 node),
   3. stores the received planes into its ghost planes (ark_set_halo),
 and the time step is the minimum over the ranks of ark_compute_dt (one all-reduce of one double).
-Every per-cell operation is the single-domain one, so the assembled state is bit-identical to the undivided run.
+Every per-cell operation is the single-domain one: the assembled state is bit-identical to the undivided run with the
+strict build of the library (-DARK_STRICT --fmad=false) and within a few ulp (1e-14 relative) with the product build,
+whose steady-state and boundary-plane code paths contract FMAs differently (tests/test_parity_gpu.py).
+
+Status: `SlabSolver` over NCCL (the batch_isend_irecv exchange, its ordering against the solver stream, the all-reduce
+of dt) has NOT run on hardware yet -- no multi-GPU box was available; what is verified is the index / exchange logic
+(gloo, CPU) and the per-rank kernels (`LocalSlabs`, one GPU).
 
 This module holds the host logic only (index arithmetic, neighbour ranks, the exchange); all arithmetic stays in the
 kernels.  `partition`, `neighbours`, `local_params` and `exchange` have no CUDA dependency and are covered by the
@@ -89,6 +95,25 @@ def exchange(dist, rank, world, periodic_z, send_lo, send_hi, recv_lo, recv_hi):
     return lo, hi
 
 
+class NonFiniteRate(RuntimeError):
+    """the CFL rate of at least one sub-domain was not finite and positive (raised on EVERY rank)."""
+
+
+def global_dt(dist, torch, local_dt, device="cpu"):
+    """Minimum of the ranks' local time steps; local_dt is None on a rank whose own rate was invalid.  Such a rank must
+    not leave before the collective (its peers would wait in the all-reduce for ever): it contributes the sentinel -1,
+    which wins the MIN against every valid (positive) step, and then every rank raises NonFiniteRate together.
+    (A NaN would not do: what MIN makes of a NaN differs between backends.)"""
+    bad = local_dt is None or not (local_dt > 0.0) or local_dt == float("inf")
+    t = torch.tensor([-1.0 if bad else float(local_dt)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN)
+    dt = float(t.item())
+    if dt < 0.0:
+        raise NonFiniteRate("ark_compute_dt: the maximum CFL rate of %s sub-domain is not finite and positive"
+                            % ("this" if bad else "another"))
+    return dt
+
+
 class SlabSolver:
     """Rank-local driver of one slab: a binding.Solver plus the halo exchange and the global time step.
 
@@ -97,7 +122,7 @@ class SlabSolver:
 
     def __init__(self, binding, prm, rank, world, dist=None, device="cuda:0"):
         import torch
-        self.torch, self.dist, self.rank, self.world = torch, dist, rank, world
+        self.torch, self.dist, self.rank, self.world, self.binding = torch, dist, rank, world, binding
         self.prm_global = dict(prm)
         self.prm, (self.k0, self.k1) = local_params(prm, rank, world)
         self.periodic = int(prm["bc_type"][2][0]) == I.BC_PERIODIC
@@ -115,12 +140,19 @@ class SlabSolver:
         return self.s.get_state()
 
     def compute_dt(self, cfl):
-        """min over the ranks of the local CFL step (= cfl / global max rate, bit-identical to the undivided domain)."""
-        dt = self.s.compute_dt(cfl)
+        """min over the ranks of the local CFL step (= cfl / global max rate, the same double as on the undivided
+        domain: a max over cells does not depend on the split).  A rank whose own rate is invalid still takes part in the
+        all-reduce (see global_dt); all ranks then raise NonFiniteRate."""
+        try:
+            dt = self.s.compute_dt(cfl)
+        except self.binding.ArkError as e:
+            if e.code != self.binding.ARK_ENONFINITE:
+                raise
+            dt = None
         if self.dist is not None and self.world > 1:
-            t = self.torch.tensor([dt], dtype=self.torch.float64, device=self.s.device)
-            self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
-            dt = float(t.item())
+            return global_dt(self.dist, self.torch, dt, self.s.device)
+        if dt is None:
+            raise NonFiniteRate("ark_compute_dt: the maximum CFL rate is not finite and positive")
         return dt
 
     def halo_exchange(self):

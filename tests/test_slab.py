@@ -125,3 +125,41 @@ def test_halo_exchange_reproduces_the_undivided_ghost_fill(world, periodic):
         assert p.exitcode == 0
     for ok, worst in res:
         assert ok == 1.0, (world, periodic, worst)
+
+
+def _dt_worker(rank, world, port, bad_rank, out):
+    sys.path.insert(0, ROOT)
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        local = [0.25, 0.125, 0.5][rank]
+        got = slab.global_dt(dist, torch, local)                            # every rank valid: the minimum, exactly
+        try:
+            slab.global_dt(dist, torch, None if rank == bad_rank else local)
+            raised = ""
+        except slab.NonFiniteRate as e:
+            raised = str(e)
+        after = slab.global_dt(dist, torch, local)                          # nobody is left behind in a collective
+        out.put((rank, got, raised, after))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,bad_rank", [(2, 1), (3, 0)])
+def test_invalid_rate_on_one_rank_raises_on_all_ranks_and_nobody_hangs(world, bad_rank):
+    """a rank whose ark_compute_dt fails must still enter the dt all-reduce, otherwise its peers hang."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_dt_worker, args=(r, world, port, bad_rank, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in range(world))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want = min([0.25, 0.125, 0.5][:world])
+    for rank, got, raised, after in res:
+        assert got == want and after == want
+        assert ("this" if rank == bad_rank else "another") in raised, (rank, raised)
