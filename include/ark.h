@@ -62,8 +62,8 @@ size_t ark_workspace_bytes(int nx, int ny, int nz);
 /* Create a solver.  nx,ny >= 4; nz >= 4 or nz == 1 (2D).  dx > 0 (uniform); gamma > 1
  * (ideal gas); g[3] constant gravity; mu, kappa >= 0 constant dynamic
  * viscosity and conductivity; low_mach_theta: 0 -> theta == 1, 1 -> eq. (13)
- * (PAPER.md:218-222, 325).  d_workspace: device memory, see above.  Errors: ARK_EINVAL (bad argument,
- * workspace too small or misaligned), ARK_ECUDA. */
+ * (PAPER.md:218-222, 325).  d_workspace: device memory of the CURRENT device, see above.  Errors: ARK_EINVAL (bad
+ * argument, workspace too small, misaligned or not memory of the current device), ARK_ECUDA. */
 int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma, const double g[3],
                double mu, double kappa, int low_mach_theta, const ark_bc* bc,
                void* d_workspace, size_t workspace_bytes, void* cuda_stream);
@@ -164,7 +164,8 @@ int ark_set_potential(ark_solver*, const double* d_phi, void* d_buffer, size_t b
  * cell sees the same neighbourhood as on the undivided domain: the assembled result is bit-identical to it in the strict
  * build (-DARK_STRICT --fmad=false) and within a few ulp (1e-14 relative) in the product build, whose steady-state and
  * boundary-plane code paths contract FMAs differently.  side: 0 = low z, 1 = high z.  Both calls are asynchronous
- * on the stream; the caller moves the buffers between devices (NCCL send/recv or peer copies over NVLink).  ark_run and
+ * on the stream; ark_get_halo is accepted on any 3D solver and side (a physical wall side simply hands out its interior
+ * planes; slab.LocalSlabs relies on it), ark_set_halo only on ARK_BC_EXTERNAL sides; the caller moves the buffers between devices (NCCL send/recv or peer copies over NVLink).  ark_run and
  * array-valued potentials are not available on sub-domains.  Errors: ARK_EINVAL (2D solver, bad side, side not
  * external), ARK_ECUDA. */
 size_t ark_halo_bytes(int nx, int ny, int nz);

@@ -153,6 +153,27 @@ def cfl_dt_static(params, U, cfl, out, stream=None):
     return out
 
 
+class _OnDevice:
+    """The library's functions, each wrapped so that it runs while `device` is the current CUDA device: a handle belongs
+    to the device that was current in ark_create (its kernel attributes, stream and workspace live there), and every entry
+    point checks that.  Without this, Solver(device="cuda:1") created while device 0 is current would record device 0."""
+
+    def __init__(self, lib, device):
+        index = torch.device(device).index
+        self._lib, self._index, self._cache = lib, (torch.cuda.current_device() if index is None else index), {}
+
+    def __getattr__(self, name):
+        fn = self._cache.get(name)
+        if fn is None:
+            raw, index = getattr(self._lib, name), self._index
+
+            def fn(*args):
+                with torch.cuda.device(index):
+                    return raw(*args)
+            self._cache[name] = fn
+        return fn
+
+
 class Solver:
     """ark_create / ark_set_state / ark_get_state / ark_compute_dt / ark_step / ark_run / ark_destroy.
 
@@ -186,11 +207,11 @@ class Solver:
                 bc.value[d][s] = float(params["bc_value"][d][s])
         g = (C.c_double * 3)(*[float(x) for x in params["g"]])
         h = C.c_void_p()
-        _check(lib.ark_create(C.byref(h), self.nx, self.ny, self.nz, float(params["dx"]), float(params["gamma"]), g,
+        self._lib = _OnDevice(lib, self.device)   # every call below runs with the solver's device current (ark.h)
+        _check(self._lib.ark_create(C.byref(h), self.nx, self.ny, self.nz, float(params["dx"]), float(params["gamma"]), g,
                               float(params["mu"]), float(params["kappa"]), int(params["theta"]), C.byref(bc),
                               C.c_void_p(self._ws_ptr), C.c_size_t(nbytes), C.c_void_p(self.stream.cuda_stream)))
         self._h = h
-        self._lib = lib
         self._phi_buf = None
         # size queries are answered once here: get_halo / set_halo run every step of a slab run
         self._halo_doubles = int(lib.ark_halo_bytes(self.nx, self.ny, self.nz)) // 8

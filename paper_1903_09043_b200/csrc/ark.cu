@@ -294,8 +294,9 @@ const char* ark_last_error(void) { return g_err; }
 
 const char* ark_version_string(void) {
     static char buf[256];
-    // ARK_KERNEL_REV names the revision of the step kernels the committed ncu counters (profiles/) belong to: bump it
-    // with every change to the kernels' arithmetic or memory traffic
+    // ARK_KERNEL_REV names the revision of the 3D step kernel (ark_k_step3) the committed ncu counters (profiles/) belong
+    // to: bump it with every change to THAT kernel's arithmetic or memory traffic (the 2D kernel has no committed counters;
+    // its changes are recorded in DESIGN.md 5.3 only)
     snprintf(buf, sizeof buf, "ark-b200 0.2 (sm_100a; K=%.2f; ng=%d; tile3d=%dx%d (%d row pairs) tile2d=%dx%d; kernels %s)", ARK_K_IMPEDANCE, ARK_NG,
              TX3, TY3, NW3, TX2, TY2, ARK_KERNEL_REV);
     return buf;
@@ -433,6 +434,15 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     if (!d_workspace || workspace_bytes < L.total || ((size_t)d_workspace & 255))
         return fail(ARK_EINVAL, "ark_create: workspace NULL, misaligned (256 B) or smaller than ark_workspace_bytes()%s");
 
+    {   // the handle lives on the CURRENT device (kernel attributes, launches): its workspace must be memory of that device
+        int dev = -1;
+        cudaPointerAttributes at;
+        ARK_CUDA(cudaGetDevice(&dev));
+        ARK_CUDA(cudaPointerGetAttributes(&at, d_workspace));
+        if ((at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) || (at.type == cudaMemoryTypeDevice && at.device != dev))
+            return fail(ARK_EINVAL, "ark_create: the workspace is not device memory of the current CUDA device (%s%lld); make the "
+                                    "workspace's device current before calling", "", (long long)dev);
+    }
     ark_solver* s = new (std::nothrow) ark_solver;
     if (!s) return fail(ARK_ENOMEM, "ark_create: out of host memory%s");
     memset(s, 0, sizeof *s);
@@ -746,6 +756,9 @@ int ark_set_potential(ark_solver* s, const double* d_phi, void* d_buffer, size_t
     ARK_ON_DEVICE(s);
     ArkParams& P = s->P;
     if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    // wall ghost cells carry the hydrostatic extrapolation for the potential that was set when they were filled
+    // (relation (14) with the potential difference): whatever sweeps already ran on the current state are stale now
+    s->xghost_valid = s->yghost_valid = s->xyghost_valid = false;
     if (d_phi && P.ndim == 3 && (P.bc[2][0] == ARK_BCK_EXTERNAL || P.bc[2][1] == ARK_BCK_EXTERNAL))
         return fail(ARK_EINVAL, "ark_set_potential: not available on a sub-domain with external ghost planes%s");
     if (!d_phi) {                                   // back to the constant gravity vector of ark_create

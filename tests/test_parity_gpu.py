@@ -567,6 +567,54 @@ def test_parity_general_path(B, name):
     assert max(err) < 1e-12, (name, err)
 
 
+def test_set_potential_invalidates_ghosts_filled_for_the_old_potential(B):
+    """ark_get_halo runs the x / y ghost sweeps and marks them done for the next step; wall ghost densities depend on the
+    potential (relation (14)), so ark_set_potential in between must make the step fill them again."""
+    (prm, U), _, kind = GENERAL["3d_phi_walls_viscous"]()
+    prm = dict(prm, g=(0.0, -0.7, -1.0))                                       # constant gravity first: other ghosts
+    phi = _phi_field(prm["nx"], prm["ny"], prm["nz"], prm["dx"], kind)
+    phi_dev = torch.as_tensor(phi, dtype=torch.float64).reshape(-1).cuda()
+    a = B.Solver(prm)
+    a.set_state(to_dev(U))
+    a.get_halo(0)                                                              # x / y sweeps with the constant g
+    a.set_potential(phi_dev)
+    a.step(1e-3)
+    got = to_np(a.get_state())
+    a.close()
+    b = B.Solver(dict(prm, phi=phi))                                           # the potential was there from the start
+    b.set_state(to_dev(U))
+    b.step(1e-3)
+    want = to_np(b.get_state())
+    b.close()
+    for f in range(5):
+        assert np.array_equal(got[f], want[f]), f
+
+
+def test_solver_on_a_device_that_is_not_current(B):
+    """A handle belongs to the device current in ark_create; the binding makes the solver's device current around every
+    call.  With one GPU: the workspace check of ark_create at least refuses host memory."""
+    import ctypes as C
+    lib = B.load()
+    prm, U = RANDOM["3d_periodic"]()
+    n = lib.ark_workspace_bytes(prm["nx"], prm["ny"], prm["nz"])
+    host = torch.empty(n + 256, dtype=torch.uint8)                             # pageable host memory, 256-aligned slice
+    ptr = (host.data_ptr() + 255) // 256 * 256
+    h = C.c_void_p()
+    g = (C.c_double * 3)(0, 0, 0)
+    bc = B.ark_bc()
+    rc = lib.ark_create(C.byref(h), prm["nx"], prm["ny"], prm["nz"], prm["dx"], prm["gamma"], g, 0.0, 0.0, 1, C.byref(bc),
+                        C.c_void_p(ptr), C.c_size_t(n), None)
+    assert rc == B.ARK_EINVAL and b"not device memory" in lib.ark_last_error()
+    if torch.cuda.device_count() > 1:
+        torch.cuda.set_device(0)
+        s = B.Solver(prm, device="cuda:1")
+        s.set_state([a.to("cuda:1") for a in to_dev(U)])
+        dt = s.compute_dt(0.4)
+        s.step(dt)
+        assert torch.cuda.current_device() == 0
+        s.close()
+
+
 def test_general_path_config_shapes(B):
     """10 steps at 1e-11 on the BASELINE recipes with the Appendix-B energy update (configs 1, 4) and with the constant
     gravity of config 4 handed over as an array Phi = -g.x (the stratified column stays the paper's workload)."""
