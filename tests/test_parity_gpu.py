@@ -328,6 +328,25 @@ def test_conservation_on_gpu(B):
     assert abs(m1 - m0) < 1e-13 * m0 and abs(e1 - e0) < 1e-13 * abs(e0)
 
 
+# SURVEY 8(d), last paragraph: "Parity runs: 10 steps, identical inputs ... for all five configs (512^3 parity may be run
+# on a 128^3 sub-size)": the BASELINE sizes themselves, every cell compared (config 1 at its full 128^2 is in CONFIGS).
+# The oracle needs ~1 min for the ten 256^3 steps on the GPU box's host, seconds for the others.
+BASELINE_SIZES = {
+    "config2_gresho_512": lambda: I.config2_gresho(512),
+    "config3_rb2d_1024x512": lambda: I.config3_rb2d(1024, 512),
+    "config4_rb3d_256": lambda: I.config4_rb3d(256),
+    "config5_convection3d_128": lambda: I.config5_convection3d(128),
+}
+
+
+@pytest.mark.parametrize("name", sorted(BASELINE_SIZES))
+def test_parity_10_steps_at_baseline_sizes(B, name):
+    prm, U = BASELINE_SIZES[name]()
+    ref, dts = O.run(prm, U, 10, cfl=0.4)
+    got = gpu_run(B, prm, U, dts)
+    check_fields(ref, got, TOL, momentum_floor(prm, ref, dts), name)
+
+
 @pytest.mark.parametrize("cfg", ["config4_256", "config5_512"])
 def test_full_size_sampled_parity(B, cfg):
     """BASELINE full sizes, the launch configuration bench.py times.  One step of U^{n+1} depends on U^n within
