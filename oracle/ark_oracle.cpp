@@ -4,7 +4,7 @@
 // step of the all-Mach, well-balanced finite-volume scheme of
 // Padioleau, Tremblin, Audit, Kestener & Kokh (arXiv 1903.09043), written
 // directly from /root/reference/PAPER.md ("PAPER.md:<line>" below) with the
-// readings A1..A20 listed in DESIGN.md.  It shares no code with the CUDA path
+// readings A1..A26 listed in DESIGN.md.  It shares no code with the CUDA path
 // under paper_1903_09043_b200/csrc/ and is only ever called from tests/,
 // __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs.
 //

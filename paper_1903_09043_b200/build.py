@@ -15,15 +15,13 @@ HEADERS = ["ark_device.cuh", "ark_step.cuh", "ark_step3d.cuh", os.path.join(".."
 # 3D: 28 outputs per row (32 lanes), ARK_NW3 row pairs per block (tile height 2 * NW3 - 4) on NW3 + 2 warps;
 # ARK_REG_RING / ARK_REG_TILE: setmaxnreg targets of the ring warpgroup and of the tile warpgroups (per scheduler:
 # 1 ring warp + 2 tile warps, REG_RING + 2 * REG_TILE <= 504: with 512 the allocation never completes)
-TILES = {"ARK_TX3": 28, "ARK_NW3": 10, "ARK_REG_RING": 72, "ARK_REG_TILE": 216, "ARK_TX2": 28, "ARK_TY2": 8,
-         "ARK_TM_GRAN": 1}
+TILES = {"ARK_TX3": 28, "ARK_NW3": 10, "ARK_REG_RING": 72, "ARK_REG_TILE": 216, "ARK_TX2": 28, "ARK_TY2": 8}
 
 
 def nvcc_cmd(out, extra=()):
-    # tile parameters can be overridden from the environment for tuning runs (ARK_NW3=10 ARK_LOW3=8 python -m ...build --force)
-    defs = ["-D%s=%d" % (k, int(os.environ.get(k, v))) for k, v in TILES.items()]
-    defs += ["-D" + d for d in os.environ.get("ARK_EXTRA_DEFS", "").split()]
-    defs += os.environ.get("ARK_EXTRA_FLAGS", "").split()          # e.g. "-Xptxas -O2" (tuning runs)
+    # the product build takes nothing from the environment: the library the tests and bench.py load is the one the
+    # committed profiles/ describe (tuning builds belong in _work/ with their own command line)
+    defs = ["-D%s=%d" % (k, v) for k, v in TILES.items()]
     return (["nvcc", "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
              "-Xcompiler", "-fPIC", "-shared", "-o", out] + defs + list(extra)
             + [os.path.join(CSRC, s) for s in SOURCES])

@@ -308,7 +308,7 @@ namespace {
 
 // Time (in plane iterations) the grid of the 3D step kernel takes when its blocks are handed out in blockIdx order (x, y,
 // then z chunk) to nsm SMs, one block per SM, each block costing its planes + ~2.5 planes of prologue.
-double g_chunk_ovh = 2.5;                                     // prologue of a chunk in plane iterations (ARK_CHUNK_OVH overrides: tuning)
+constexpr double g_chunk_ovh = 2.5;                           // prologue of a chunk in plane iterations (fitted, profiles/r02_step_kernel.md)
 double chunk_makespan(long long ncol, const int* chunk, int nchunk, int nsm) {
     std::vector<double> heap((size_t)nsm, 0.0);               // min-heap of the SMs' finish times
     auto cmp = [](double a, double b) { return a > b; };
@@ -327,7 +327,6 @@ double chunk_makespan(long long ncol, const int* chunk, int nchunk, int nsm) {
 // nchunk 1..16 x ratio 1 .. 0.4, scored by the scheduling simulation above.  zb[0..nchunk] = chunk boundaries.
 int choose_zchunks(int nx, int ny, int nz, int nsm, int* zb) {
     const long long ncol = (long long)((nx + TX3 - 1) / TX3) * ((ny + TY3 - 1) / TY3);
-    if (const char* e = getenv("ARK_CHUNK_OVH")) { const double v = atof(e); if (v > 0.0) g_chunk_ovh = v; }
     const double ratios[7] = {1.0, 0.9, 0.8, 0.7, 0.6, 0.5, 0.4};
     int best[ARK_MAX_ZCHUNKS] = {nz}, nbest = 1;
     double best_t = 1e300;
@@ -477,11 +476,6 @@ int ark_create(ark_solver** out, int nx, int ny, int nz, double dx, double gamma
     if (step_blocks(nx, ny, nz, &s->step_grid, s->P.zb, nsm) > MAX_SCRATCH - DIAG_BLOCKS * ARK_NDIAG) {
         delete s;
         return fail(ARK_EINVAL, "ark_create: grid too large for the per-block rate scratch (ark_workspace_bytes returns 0 for it)%s");
-    }
-    if (ndim == 3 && getenv("ARK_DEBUG_CHUNKS")) {
-        fprintf(stderr, "ark_create: %d SMs, grid %u x %u x %u, z chunks:", nsm, s->step_grid.x, s->step_grid.y, s->step_grid.z);
-        for (unsigned c = 0; c < s->step_grid.z; ++c) fprintf(stderr, " %d", P.zb[c + 1] - P.zb[c]);
-        fprintf(stderr, "\n");
     }
     if (ndim == 3) {
         for (int b = 0; b < 2; ++b) {

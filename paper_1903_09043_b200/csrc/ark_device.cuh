@@ -170,11 +170,9 @@ ARK_DEV void ark_mbar_wait(unsigned long long* bar, unsigned parity) {
 // used; ark_tm_wait_st() orders earlier stores before later loads of the same columns.
 // ------------------------------------------------------------------------------------------------
 #ifndef ARK_HOST_EMU
-// ARK_TM_CLOBBER: "memory" makes every TMEM transfer a scheduling fence for shared / global accesses (TMEM is not
-// memory the compiler knows about: the volatile asm statements keep their own relative order)
-#ifndef ARK_TM_CLOBBER
+// The "memory" clobber makes every TMEM transfer a scheduling fence for shared / global accesses (TMEM is not memory the
+// compiler knows about: the volatile asm statements keep their own relative order)
 #define ARK_TM_CLOBBER "memory"
-#endif
 #define ARK_LO(x) "r"(__double2loint(x))
 #define ARK_HI(x) "r"(__double2hiint(x))
 ARK_DEV unsigned ark_tm_alloc_all(unsigned* slot_in_smem) {           // one full warp; 512 columns = the whole TMEM
@@ -200,63 +198,21 @@ ARK_DEV void ark_tm_ld2(unsigned a, double& v0, double& v1) {
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1);
 }
-// ARK_TM_GRAN: doubles moved per tcgen05 instruction.  Wide transfers need their 2*GRAN registers contiguous, which
-// costs register-packing moves; narrow ones cost more tcgen05 instructions.
-#ifndef ARK_TM_GRAN
-#define ARK_TM_GRAN 8
-#endif
-#if ARK_TM_GRAN >= 4
-ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(a), ARK_LO(v0), ARK_HI(v0), ARK_LO(v1),
-                 ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3) : ARK_TM_CLOBBER);
-}
-#elif ARK_TM_GRAN == 2
-ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) { ark_tm_st2(a, v0, v1); ark_tm_st2(a + 4, v2, v3); }
-#else
+// Wider groups go as single-double transfers: x8 / x16 tcgen05 shapes need their 8 / 16 registers contiguous, and the
+// register-packing moves that costs were measured to outweigh the saved instructions (profiles/r02_step_kernel.md).
 ARK_DEV void ark_tm_st4(unsigned a, double v0, double v1, double v2, double v3) { ark_tm_st1(a, v0); ark_tm_st1(a + 2, v1); ark_tm_st1(a + 4, v2); ark_tm_st1(a + 6, v3); }
-#endif
-#if ARK_TM_GRAN >= 8
-ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
-    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(a),
-                 ARK_LO(v0), ARK_HI(v0), ARK_LO(v1), ARK_HI(v1), ARK_LO(v2), ARK_HI(v2), ARK_LO(v3), ARK_HI(v3), ARK_LO(v4), ARK_HI(v4),
-                 ARK_LO(v5), ARK_HI(v5), ARK_LO(v6), ARK_HI(v6), ARK_LO(v7), ARK_HI(v7) : ARK_TM_CLOBBER);
-}
-#else
 ARK_DEV void ark_tm_st8(unsigned a, double v0, double v1, double v2, double v3, double v4, double v5, double v6, double v7) {
     ark_tm_st4(a, v0, v1, v2, v3); ark_tm_st4(a + 8, v4, v5, v6, v7);
 }
-#endif
 ARK_DEV void ark_tm_ld1(unsigned a, double& v0) {
     int l0, h0;
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0,%1}, [%2];" : "=r"(l0), "=r"(h0) : "r"(a) : ARK_TM_CLOBBER);
     v0 = __hiloint2double(h0, l0);
 }
-#if ARK_TM_GRAN >= 4
-ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) {
-    int l0, h0, l1, h1, l2, h2, l3, h3;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3) : "r"(a) : ARK_TM_CLOBBER);
-    v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
-}
-#elif ARK_TM_GRAN == 2
-ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) { ark_tm_ld2(a, v0, v1); ark_tm_ld2(a + 4, v2, v3); }
-#else
 ARK_DEV void ark_tm_ld4(unsigned a, double& v0, double& v1, double& v2, double& v3) { ark_tm_ld1(a, v0); ark_tm_ld1(a + 2, v1); ark_tm_ld1(a + 4, v2); ark_tm_ld1(a + 6, v3); }
-#endif
-#if ARK_TM_GRAN >= 8
-ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
-    int l0, h0, l1, h1, l2, h2, l3, h3, l4, h4, l5, h5, l6, h6, l7, h7;
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                 : "=r"(l0), "=r"(h0), "=r"(l1), "=r"(h1), "=r"(l2), "=r"(h2), "=r"(l3), "=r"(h3), "=r"(l4), "=r"(h4), "=r"(l5), "=r"(h5),
-                   "=r"(l6), "=r"(h6), "=r"(l7), "=r"(h7) : "r"(a) : ARK_TM_CLOBBER);
-    v0 = __hiloint2double(h0, l0); v1 = __hiloint2double(h1, l1); v2 = __hiloint2double(h2, l2); v3 = __hiloint2double(h3, l3);
-    v4 = __hiloint2double(h4, l4); v5 = __hiloint2double(h5, l5); v6 = __hiloint2double(h6, l6); v7 = __hiloint2double(h7, l7);
-}
-#else
 ARK_DEV void ark_tm_ld8(unsigned a, double& v0, double& v1, double& v2, double& v3, double& v4, double& v5, double& v6, double& v7) {
     ark_tm_ld4(a, v0, v1, v2, v3); ark_tm_ld4(a + 8, v4, v5, v6, v7);
 }
-#endif
 #endif
 
 // ------------------------------------------------------------------------------------------------

@@ -87,7 +87,6 @@ struct ArkMarch3 {
     int tx, ty;                          // box origin in the padded array (columns, rows)
     unsigned long long* mbar;            // the block's three mbarriers (one per UR slot)
     unsigned phase;                      // parity bit of each slot's next completion
-    unsigned bphase;                     // parity of the next completion of barrier B (split arrive / wait)
     double* Ocur;                        // row a, plane q-1 of the output state (row b: + px)
     long long pstride, fs;
     int px;
@@ -140,44 +139,21 @@ ARK_DEV void ark_ring_wait3(ArkMarch3<VISC, TX, NW>& M, int slot) {
 #endif
 }
 
-// Block barrier (B) of a plane.  ARK_SPLIT_B == 1 makes it a SPLIT barrier: every warp arrives (one elected lane, after
-// __syncwarp, on an mbarrier that counts warps) as soon as its faces / differences / primitives are in shared memory, goes
-// on with work that only needs its own data (the parked z pipeline, five of the six dissipative face fluxes) and waits
-// right before it reads a neighbour's.  Measured on B200 (512^3): 5.367 ms split vs 5.356 ms with the plain
-// __syncthreads at the arrive point -- no gain, so the product build keeps the plain barrier (ARK_SPLIT_B == 0); the
-// reordering that the split needs (independent work first) is kept, it alone gave 1.4 %.
-// ARK_UNROLL2 == 1 unrolls the steady plane loop twice (alternating slots become compile-time constants, 1198 -> 1150
-// static instructions per plane).  Measured on B200: 5.60 ms vs 5.14 ms at 512^3 -- the hot loops of the four roles
-// (18 + 5 + 6.6 + 1.3 KB) just fit the 32 KB L1.5 instruction cache, the unrolled tile loop (37 KB) does not.  Off.
-#ifndef ARK_UNROLL2
-#define ARK_UNROLL2 0
-#endif
+// Block barrier (B) of a plane: a plain __syncthreads at the point where a warp's faces / differences / primitives are in
+// shared memory; work that only needs the warp's own data (the parked z pipeline, five of the six dissipative face fluxes)
+// is ordered BEFORE it.  Measured and rejected (profiles/r02_step_kernel.md): a split arrive / wait on an mbarrier
+// (5.367 vs 5.356 ms at 512^3) and unrolling the steady plane loop twice (5.60 vs 5.14 ms: the unrolled tile loop, 37 KB,
+// no longer fits the 32 KB instruction cache).
 #ifndef ARK_RING_EARLY
 #define ARK_RING_EARLY 1
 #endif
-#ifndef ARK_SPLIT_B
-#define ARK_SPLIT_B 0
-#endif
 template <bool VISC, int TX, int NW>
 ARK_DEV void ark_bar_arrive(ArkMarch3<VISC, TX, NW>& M) {
-#if !defined(ARK_HOST_EMU) && ARK_SPLIT_B
-    __syncwarp();
-    if ((threadIdx.x & 31) == 0)
-        asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(ark_smem_u32(M.mbar + 4)) : "memory");
-#else
     (void)M;
     __syncthreads();
-#endif
 }
 template <bool VISC, int TX, int NW>
-ARK_DEV void ark_bar_wait(ArkMarch3<VISC, TX, NW>& M) {
-#if !defined(ARK_HOST_EMU) && ARK_SPLIT_B
-    ark_mbar_wait(M.mbar + 4, M.bphase);
-    M.bphase ^= 1u;
-#else
-    (void)M;
-#endif
-}
+ARK_DEV void ark_bar_wait(ArkMarch3<VISC, TX, NW>& M) { (void)M; }   // (the point where a neighbour's data is first read)
 
 template <bool VISC, int TX, int NW>
 ARK_DEV ArkPrim ark_march_prims3(const ArkParams& P, const ArkMarch3<VISC, TX, NW>& M, int col, int slot) {
@@ -844,13 +820,6 @@ template <bool VISC, bool GXY, bool GEN, int TX, int NW, int ROLE>
 ARK_DEV void ark_march3(const ArkParams& P, const ArkStepConst& K, ArkMarch3<VISC, TX, NW>& M) {
     int q = M.k0 - 1;
     for (; q <= M.k0; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, false>(P, K, M, q);   // k0-1, k0
-#if ARK_UNROLL2
-    // k0+1 .. k1-1, two planes per trip: at q = k0+1 the alternating slots are back at 0 (two planes after the prologue)
-    for (; q + 1 < M.k1; q += 2) {
-        ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, true, 0>(P, K, M, q);
-        ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, true, 1>(P, K, M, q + 1);
-    }
-#endif
     for (; q < M.k1; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, true>(P, K, M, q);     // k0+1 .. k1-1
     for (; q <= M.k1; ++q) ark_plane3<VISC, GXY, GEN, TX, NW, ROLE, false>(P, K, M, q);   // k1
 }
@@ -1018,13 +987,11 @@ ARK_DEV void ark_step3d_pairs(const ArkParams& P, const double* __restrict__ Uin
     M.tx = (int)(blockIdx.x * TX) - 2 + ARK_XOFF;
     M.ty = (int)(blockIdx.y * TY) - 2 + ARK_NG;
     M.phase = 0;
-    M.bphase = 0;
     unsigned tmem_base = 0;
 #ifndef ARK_HOST_EMU
     unsigned* tm_slot = (unsigned*)(smem + C::MBAR_OFF + 3);
     if (t == 0) {
         for (int s3 = 0; s3 < 3; ++s3) ark_mbar_init(M.mbar + s3, 1);
-        ark_mbar_init(M.mbar + 4, C::NWARP);          // barrier B: one arrival per warp
         ark_mbar_fence_init();
     }
     if (t < 32) ark_tm_alloc_all(tm_slot);            // the whole TMEM of the SM (one block per SM)

@@ -900,3 +900,26 @@ def test_ke_spectrum_parseval_single_mode_and_brute_force():
     E1 = O.ke_spectrum(prm, [one, one * u[None], 0 * one, 0 * one, one])
     expect = np.zeros(E.size); expect[4] = a * a / 4
     assert np.abs(E1 - expect).max() < 1e-15
+
+
+def test_oracle_is_clean_under_asan_ubsan(tmp_path):
+    """SURVEY section 5 (sanitizer row): oracle/ark_oracle.cpp built into a stand-alone executable with
+    -fsanitize=address,undefined and run on small 2D / 3D cases with every wall kind, the three energy forms and an
+    array-valued potential (tests/oracle_sanitizer_main.cpp).  Any out-of-bounds access, use of an uninitialised vector
+    slot beyond its size, signed overflow or misaligned access aborts the run (-fno-sanitize-recover)."""
+    import shutil
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if shutil.which("g++") is None:
+        pytest.skip("no g++")
+    exe = str(tmp_path / "oracle_asan")
+    cmd = ["g++", "-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+           "-o", exe, os.path.join(root, "tests", "oracle_sanitizer_main.cpp"), os.path.join(root, "oracle", "ark_oracle.cpp")]
+    b = subprocess.run(cmd, capture_output=True, text=True)
+    if b.returncode != 0 and ("asan" in b.stderr or "ubsan" in b.stderr or "sanitize" in b.stderr):
+        pytest.skip("sanitizer runtime not installed: " + b.stderr.strip().splitlines()[-1])
+    assert b.returncode == 0, b.stderr
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=300,
+                       env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1"))
+    assert r.returncode == 0, (r.stdout, r.stderr)
+    assert r.stdout.count(" ok ") == 5 and "ERROR" not in r.stderr and "runtime error" not in r.stderr, (r.stdout, r.stderr)
