@@ -8,8 +8,10 @@ columns are written by the step kernel itself), fused acoustic+transport+dissipa
 epilogue, the second reduction pass and the 16-byte device->host read of dt (ark_compute_dt) -- exactly the loop
 {dt = ark_compute_dt(cfl); ark_step(dt)}.
 
-The JSON line of the default workload (config5_512) also carries, under "also", the same measurement of the other
-roofline target of north_star (config4_256).  The fp64 peak of the "alu" roofline is MEASURED in the same run
+The JSON line of the default workload (config5_512) also carries, under "also" (a list), the same measurement of the other
+roofline target of north_star (config4_256), of the kernel variants no BASELINE config selects (inviscid3d_512: <VISC=0>;
+config4_256_phi: the general path with an array-valued potential, 88 B per cell update) and of the three 2D BASELINE
+configs (host loop and ark_run), each with its own clocks record.  The fp64 peak of the "alu" roofline is MEASURED in the same run
 (ark_measure_fp64_peak: DFMA chains); the ncu-derived per-cell counters come from profiles/r02_step_kernel_counters.csv
 and are only reported when that file was captured for the kernel revision of the loaded library.
 
@@ -40,7 +42,14 @@ WORKLOADS = {
     "config3_1024x512": ("config3_rb2d", (1024, 512), 64, (512, 256)),
     "config2_512": ("config2_gresho", 512, 64, 512),
     "config1_128": ("config1_atmosphere", 128, 64, 128),
+    # kernel variants that no BASELINE config selects (they ride along under "also"): the Euler part
+    # alone (<VISC=0>) and the general path with an array-valued potential (<GEN=1>, 88 B per cell update)
+    "inviscid3d_512": ("inviscid_convection3d", 512, 80, 256),
+    "config4_256_phi": ("config4_rb3d_phi", 256, 88, 128),
 }
+# measured in the same line as the default workload: (name, timed steps of the host loop, ark_run steps or 0)
+ALSO = [("config4_256", 20, 0), ("inviscid3d_512", 10, 0), ("config4_256_phi", 20, 0),
+        ("config3_1024x512", 200, 2000), ("config2_512", 200, 2000), ("config1_128", 200, 2000)]
 
 
 def build_workload(name, device=None, sample=False):
@@ -233,7 +242,7 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def measure_workload(name, K, W, dev, local, world, dist, e2e=True):
+def measure_workload(name, K, W, dev, local, world, dist, e2e=True, run_steps=0):
     """K timed steps of {compute_dt; step} of one workload (after W warm-up steps), device-timed on the solver's
     stream, max over ranks; the step kernel's own time from events the library records around its launches; optionally
     the end-to-end variant with HOST buffers.  Returns a dict of raw numbers."""
@@ -249,6 +258,8 @@ def measure_workload(name, K, W, dev, local, world, dist, e2e=True):
     U = [None if a is None else a.reshape(-1).contiguous() for a in U]
     ncell = prm["nx"] * prm["ny"] * prm["nz"]
     s = binding.Solver(prm, device=dev)
+    gen = prm.get("phi") is not None
+    prm = {k: v for k, v in prm.items() if k != "phi"}      # (the solver holds its padded copy; drop the dense one)
     s.set_state(U)
     for _ in range(W):
         s.step(s.compute_dt(CFL))
@@ -272,11 +283,29 @@ def measure_workload(name, K, W, dev, local, world, dist, e2e=True):
     s.step_kernel_timing(False)
     launches = s.launch_count() - l0
     ms_total = max_over_ranks(ms_total, dist, dev)
-    out = {"prm": prm, "bpc": bpc, "ncell": ncell, "ms_total": ms_total, "kern_ms": kern_ms, "kern_n": kern_n,
+    visc = prm["mu"] > 0 or prm["kappa"] > 0
+    out = {"variant": "<VISC=%d,GXY=%d,GEN=%d>" % (visc, gen or prm["g"][0] != 0 or prm["g"][1] != 0, gen) if prm["nz"] > 1
+                      else "<2,VISC=%d,GEN=%d>" % (visc, gen),
+           "prm": prm, "bpc": bpc, "ncell": ncell, "ms_total": ms_total, "kern_ms": kern_ms, "kern_n": kern_n,
            "launches": launches, "clocks": clocks, "value": whole_job_value(world, ncell, K, ms_total * 1e-3)}
 
     # sanity: state still finite after the timed steps
     assert s.compute_dt(CFL) > 0
+
+    if run_steps > 0:
+        # ---- the same steps through ark_run: dt stays on the device, pairs of steps replayed from a CUDA graph (the 2D
+        # configs are launch-latency-bound; this is the loop a user of the library would run)
+        s.run(8, CFL)
+        l1 = s.launch_count()
+        barrier()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        s.run(run_steps, CFL)
+        r1.record()
+        barrier()
+        run_ms = max_over_ranks(r0.elapsed_time(r1), dist, dev)
+        out["ark_run"] = {"steps": run_steps, "us_per_step": run_ms / run_steps * 1e3, "value": whole_job_value(world, ncell, run_steps, run_ms * 1e-3),
+                          "unit": UNIT, "gpu_launches": s.launch_count() - l1}
 
     if e2e:
         # ---- end to end through the C ABI with HOST buffers (pinned): set_state_host + compute_dt + step + get_state_host
@@ -352,7 +381,7 @@ def roofline_objects(name, m, world, version, fp64_peak):
     kern_avg_ms = m["kern_ms"] / max(m["kern_n"], 1)
     achieved = alg_bytes / (kern_avg_ms * 1e-3) / 1e9
     c = counters_for(name, version)
-    hbm = {"bound": "hbm", "kernel": "ark_k_step3" if m["prm"]["nz"] > 1 else "ark_k_step", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    hbm = {"bound": "hbm", "kernel": ("ark_k_step3" if m["prm"]["nz"] > 1 else "ark_k_step") + m["variant"], "achieved": achieved, "peak": peak, "unit": "GB/s",
            "frac": achieved / peak, "traffic": c["dram_bytes_per_launch"] if c else None,
            "traffic_from": c["source"] if c else "no ncu capture of kernel revision %s in profiles/" % kernel_rev(version),
            "peak_source": peak_src, "algorithmic_bytes_per_cell": m["bpc"], "kernel_ms": kern_avg_ms,
@@ -404,10 +433,12 @@ def run_ours(args):
         return
     m = measure_workload(args.workload, K, W, dev, local, world, dist, e2e=not args.no_e2e)
     fp64_peak = binding.measure_fp64_peak()
-    also = None
+    also = []
     if args.workload == "config5_512" and not args.no_also:
-        # the other roofline target of north_star, same measurement, in the same driver-run line
-        also = ("config4_256", measure_workload("config4_256", max(K, 20), W, dev, local, world, dist, e2e=False))
+        # the other roofline target of north_star (config4_256), the kernel variants no BASELINE config selects and the
+        # three 2D BASELINE configs: same measurement, same driver-run line, each with its own clocks record
+        for name2, k2, run2 in ALSO:
+            also.append((name2, measure_workload(name2, k2, W, dev, local, world, dist, e2e=False, run_steps=run2)))
 
     if rank == 0:
         prm, bpc, ncell = m["prm"], m["bpc"], m["ncell"]
@@ -422,13 +453,17 @@ def run_ours(args):
                            "parallelism": "replicas only" if world > 1 else "single GPU",
                            "library": version},
                 "roofline": hbm, "roofline_fp64": alu, "e2e": m.get("e2e"), "gpu_launches": m["launches"], "clocks": m["clocks"]}
-        if also is not None:
-            name2, m2 = also
-            hbm2, alu2 = roofline_objects(name2, m2, world, version, fp64_peak)
-            k2 = m2["kern_n"]
-            line["also"] = {"workload": name2, "grid": [m2["prm"]["nx"], m2["prm"]["ny"], m2["prm"]["nz"]], "steps": k2,
-                            "value": m2["value"], "unit": UNIT, "ms_per_step": m2["ms_total"] / k2, "roofline": hbm2,
-                            "roofline_fp64": alu2, "gpu_launches": m2["launches"], "clocks": m2["clocks"]}
+        if also:
+            line["also"] = []
+            for name2, m2 in also:
+                hbm2, alu2 = roofline_objects(name2, m2, world, version, fp64_peak)
+                k2 = m2["kern_n"]
+                ent = {"workload": name2, "grid": [m2["prm"]["nx"], m2["prm"]["ny"], m2["prm"]["nz"]], "steps": k2,
+                       "value": m2["value"], "unit": UNIT, "ms_per_step": m2["ms_total"] / k2, "roofline": hbm2,
+                       "roofline_fp64": alu2, "gpu_launches": m2["launches"], "clocks": m2["clocks"]}
+                if "ark_run" in m2:
+                    ent["ark_run"] = m2["ark_run"]
+                line["also"].append(ent)
         if world == 1 and not args.no_cpu_baseline:
             val, ms, sample = oracle_timed(args.workload, 2, 0)
             line["cpu_baseline"] = cpu_baseline_record(val, sample)
@@ -461,7 +496,7 @@ def main():
                     help="N > 1: independent replicas (default, north_star: the path does not shard) or ONE workload split along z (slab.py)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (kernel tuning runs)")
-    ap.add_argument("--no-also", action="store_true", help="skip the config4_256 measurement that rides along with config5_512")
+    ap.add_argument("--no-also", action="store_true", help="skip the other workloads that ride along with config5_512")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -264,6 +264,23 @@ def config5_convection3d(n=512, seed=1005, amp=1e-2, theta=1, device=None, box=N
     return _convection3d(n, n, 1.0, 100.0, 1.0e-4, 2.5e-4, BC_REFLECTING, amp, seed, theta, device, box, heat=heat)
 
 
+def inviscid_convection3d(n=512, seed=1005, amp=1e-2, theta=1, device=None, box=None):
+    """Measurement workload (bench.py `inviscid3d_512`): the config-5 stratification and noise WITHOUT dissipation
+    (mu = kappa = 0, reflecting walls on both z sides), i.e. the Euler part of the scheme alone: the 3D step kernel's
+    <VISC=0> instantiation, 80 B per cell update."""
+    return _convection3d(n, n, 1.0, 100.0, 0.0, 0.0, BC_REFLECTING, amp, seed, theta, device, box, heat=0.0)
+
+
+def config4_rb3d_phi(n=256, seed=1004, amp=1e-3, theta=1, device=None):
+    """Measurement workload (bench.py `config4_256_phi`): BASELINE config 4 with its constant gravity g = (0,0,-1) handed
+    over as the array-valued potential Phi = -g.x at the cell centres: the general path of the step kernel
+    (88 B per cell update: the potential is read as a sixth field)."""
+    prm, U = config4_rb3d(n, seed=seed, amp=amp, theta=theta, device=device)
+    zc = (np.arange(n) + 0.5) * prm["dx"]
+    prm = dict(prm, phi=_full(_col(zc, 2, device), n, n, n, device))
+    return prm, U
+
+
 # --------------------------------------------------------------------------- second workloads (SURVEY 8(f) row 3)
 def rayleigh_taylor(nx=200, ny=600, C=0.01, theta=1, mu=0.0, device=None):
     """Rayleigh-Taylor test case: domain [-0.25,0.25] x [-0.75,0.75] (L_x = 0.5, L_y = 1.5), rho = 1
