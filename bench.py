@@ -12,7 +12,7 @@ The JSON line of the default workload (config5_512) also carries, under "also" (
 roofline target of north_star (config4_256), of the kernel variants no BASELINE config selects (inviscid3d_512: <VISC=0>;
 config4_256_phi: the general path with an array-valued potential, 88 B per cell update) and of the three 2D BASELINE
 configs (host loop and ark_run), each with its own clocks record.  The fp64 peak of the "alu" roofline is MEASURED in the same run
-(ark_measure_fp64_peak: DFMA chains); the ncu-derived per-cell counters come from profiles/r02_step_kernel_counters.csv
+(ark_measure_fp64_peak: DFMA chains); the ncu-derived per-cell counters come from profiles/r03_step_kernel_counters.csv
 and are only reported when that file was captured for the kernel revision of the loaded library.
 
 Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs N independent
@@ -67,7 +67,7 @@ def build_workload(name, device=None, sample=False):
 # fp64 ALU roof: measured in the same run by a register-resident DFMA-chain kernel of the library
 # (ark_measure_fp64_peak).  For context: 64 fp64 instructions / clk / SM x 148 SMs x 1965 MHz = 18.61 T instr/s nominal.
 FP64_INSTR_PER_CLK_SM, N_SM, SM_MAX_MHZ = 64, 148, 1965.0
-COUNTERS_CSV = os.path.join(ROOT, "profiles", "r02_step_kernel_counters.csv")
+COUNTERS_CSV = os.path.join(ROOT, "profiles", "r03_step_kernel_counters.csv")
 
 
 def kernel_rev(version_string):

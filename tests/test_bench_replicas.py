@@ -72,7 +72,7 @@ def test_single_process_path_needs_no_process_group():
 
 
 def test_ncu_counters_in_profiles_belong_to_the_built_kernels():
-    """bench.py prints roofline.traffic and fp64 instructions per cell from profiles/r02_step_kernel_counters.csv; the
+    """bench.py prints roofline.traffic and fp64 instructions per cell from profiles/r03_step_kernel_counters.csv; the
     rows must have been captured for the kernel revision the library reports (ark_version_string needs no GPU), and a
     row of another revision must be ignored instead of being printed as if it were current."""
     sys.path.insert(0, ROOT)
@@ -82,14 +82,16 @@ def test_ncu_counters_in_profiles_belong_to_the_built_kernels():
     rev = bench.kernel_rev(version)
     assert rev, version
     table = bench.load_counters()
-    for name in ("config5_512", "config4_256"):
+    cells = {"config5_512": (512 ** 3, 80.0), "config4_256": (256 ** 3, 80.0), "inviscid3d_512": (512 ** 3, 80.0),
+             "config4_256_phi": (256 ** 3, 88.0)}
+    for name in sorted(cells):
         assert name in table, "no ncu counters committed for %s" % name
         assert table[name]["kernel_rev"] == rev, (name, table[name]["kernel_rev"], rev)
         assert os.path.exists(os.path.join(ROOT, table[name]["source"]))
         c = bench.counters_for(name, version, table)
         assert c is not None and 200.0 < c["fp64_instr_per_cell"] < 600.0
-        ncell = {"config5_512": 512 ** 3, "config4_256": 256 ** 3}[name]
-        assert 1.0 <= c["dram_bytes_per_launch"] / (80.0 * ncell) < 1.3          # DRAM traffic close to the algorithmic 80 B/cell
+        ncell, bpc = cells[name]
+        assert 1.0 <= c["dram_bytes_per_launch"] / (bpc * ncell) < 1.3           # DRAM traffic close to the algorithmic bytes per cell
     stale = {"config5_512": dict(table["config5_512"], kernel_rev="r0.0")}
     assert bench.counters_for("config5_512", version, stale) is None
 
