@@ -163,29 +163,33 @@ def test_hydrostatic_atmosphere_stays_at_rest(B):
 
 
 def test_uniform_state_is_preserved(B):
-    """A constant state (u* = u, Pi* = p, L~ = 1, every flux difference vanishes) stays constant.
-    The 2D kernel forms all flux differences of a cell at once and is bit-exact.  The 3D kernel applies a face flux
-    as soon as it is known (the high-z and high-y fluxes of a cell arrive one plane later), so +lam F and -lam F are
-    rounded separately: the state is preserved to a few ulp instead."""
+    """A constant state (u* = u, Pi* = p, L~ = 1, every flux difference vanishes) stays constant:
+    bit for bit in 2D and in the inviscid 3D kernel.  The viscous 3D kernel applies a face flux as soon as it is known
+    (the high-z and high-y fluxes of a cell arrive one plane later), so +lam F and -lam F are rounded separately:
+    measured <= 3 ulp (rho v), <= 1 ulp (rho w, E), exact (rho, rho u), the same after 5 and after 100 steps -- a
+    fixed point of the rounding, not a drift (reading A27 of DESIGN.md).  Asserted: <= 4 ulp after 5 and after 50 steps."""
     for shape in ((1, 20, 40), (12, 20, 40), (40, 37, 61)):
-        nz, ny, nx = shape
-        prm = I.make_params(nx, ny, nz, 0.1, 1.4, mu=0.01, kappa=0.02)
-        rho, u, v, w, p = 1.25, 0.5, -0.25, (0.125 if nz > 1 else 0.0), 0.75
-        E = p / 0.4 + 0.5 * rho * (u * u + v * v + w * w)
-        U = [np.full(shape, x) for x in (rho, rho * u, rho * v, rho * w, E)]
-        if nz == 1:
-            U[3] = None
-        s = B.Solver(prm)
-        s.set_state(to_dev(U))
-        s.run(5, 0.4)
-        out = to_np(s.get_state())
-        s.close()
-        for f in range(5):
-            if out[f] is not None:
-                if nz == 1:
-                    assert np.array_equal(out[f], U[f].reshape(-1)), f
-                else:
-                    assert np.abs(out[f] - U[f].reshape(-1)).max() <= 5 * 4 * np.spacing(np.abs(U[f]).max()), f
+        for mu, kappa in ((0.01, 0.02), (0.0, 0.0)):
+            nz, ny, nx = shape
+            prm = I.make_params(nx, ny, nz, 0.1, 1.4, mu=mu, kappa=kappa)
+            rho, u, v, w, p = 1.25, 0.5, -0.25, (0.125 if nz > 1 else 0.0), 0.75
+            E = p / 0.4 + 0.5 * rho * (u * u + v * v + w * w)
+            U = [np.full(shape, x) for x in (rho, rho * u, rho * v, rho * w, E)]
+            if nz == 1:
+                U[3] = None
+            s = B.Solver(prm)
+            s.set_state(to_dev(U))
+            for nsteps in (5, 45):
+                s.run(nsteps, 0.4)
+                out = to_np(s.get_state())
+                for f in range(5):
+                    if out[f] is None:
+                        continue
+                    if nz == 1 or mu == 0.0:
+                        assert np.array_equal(out[f], U[f].reshape(-1)), (shape, mu, f)
+                    else:
+                        assert np.abs(out[f] - U[f].reshape(-1)).max() <= 4 * np.spacing(np.abs(U[f]).max()), (shape, f)
+            s.close()
 
 
 def test_ghost_fill_matches_oracle(B):
@@ -208,6 +212,39 @@ def test_ghost_fill_matches_oracle(B):
     s.close()
     for f in range(5):
         assert np.array_equal(got[f], np.pad(U[f], 2, mode="wrap"))
+
+
+def test_step_kernels_leave_periodic_ghosts_behind(B):
+    """Periodic grids: the step kernels write the x ghost columns of the state they produce (2D, periodic x and y: the y
+    ghost rows and corners too), so a step launches pass 2 + y sweep + z sweep + step kernel = 4 kernels in 3D and
+    pass 2 + step kernel = 2 in 2D.  After some steps the padded planes must be the periodic wrap of the interior, bit
+    for bit (ragged tiles, several y tiles, wrapped columns / rows in the first and the last tile).  (Writing the y ghost
+    rows from the 3D kernel as well was measured and rejected, profiles/r03_kernel_variants.md.)"""
+    cases = [(I.random_state(45, 21, 19, 5, g=(0, 0, -1.0), mu=1e-3, kappa=2e-3,
+                             bc_type=((PER, PER), (PER, PER), (REF, REF))), 4),
+             (I.random_state(61, 40, 12, 8, bc_type=((PER, PER), (PER, PER), (PER, PER))), 4),
+             (I.random_state(70, 37, 1, 3), 2)]
+    for (prm, U), per_step in cases:
+        s = B.Solver(prm)
+        s.set_state(to_dev(U))
+        for _ in range(3):
+            s.step(s.compute_dt(0.4))
+        l0 = s.launch_count()
+        for _ in range(4):
+            s.step(s.compute_dt(0.4))
+        assert s.launch_count() - l0 == 4 * per_step, (prm["nz"], s.launch_count() - l0)
+        l1 = s.launch_count()
+        pad = to_np(s.get_padded())                          # 3D: y and z sweeps + 5 copies; 2D: 4 copies, no sweep at all
+        assert s.launch_count() - l1 == (7 if prm["nz"] > 1 else 4)
+        inner = to_np(s.get_state())
+        s.close()
+        for f in range(5):
+            if pad[f] is None:
+                continue
+            a = inner[f].reshape(prm["nz"], prm["ny"], prm["nx"])
+            want = np.pad(a, ((0, 0), (2, 2), (2, 2)), mode="wrap")
+            got = pad[f][2:-2] if prm["nz"] > 1 else pad[f]
+            assert np.array_equal(got, want), (prm["nz"], f)
 
 
 def test_compute_dt_and_run_match_oracle(B):
