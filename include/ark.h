@@ -125,6 +125,16 @@ int ark_cfl_dt_static(int nx, int ny, int nz, double dx, double gamma, double mu
  * fluxes, conservative update).  Asynchronous on the stream. */
 int ark_step(ark_solver*, double dt);
 
+/* The two halves of { ark_compute_dt ; ark_step } with the numbers kept in DEVICE memory, for time loops in which the step
+ * size depends on more than this solver and the host must not wait for the GPU: a slab decomposition
+ * takes dt = cfl / (max over the sub-domains' maximum rates), which a collective can form on device memory.
+ * ark_max_rate_device writes the maximum CFL rate of the current state (the quantity ark_compute_dt divides cfl by) to
+ * d_rate_out (1 double); ark_step_device_dt advances the state by the step size found in d_dt (1 double) when the
+ * kernels run.  Both are asynchronous on the stream and check nothing on the host: a rate that is not finite and positive
+ * simply propagates (NaN state); call ark_compute_dt from time to time to detect that.  Errors: ARK_EINVAL, ARK_ECUDA. */
+int ark_max_rate_device(ark_solver*, double* d_rate_out);
+int ark_step_device_dt(ark_solver*, const double* d_dt);
+
 /* Convenience: nsteps x { dt = cfl / max rate ; step(dt) } with the time step kept on the device
  * (no host round trip per step).  If dts_out (HOST, nsteps doubles) is not NULL the step sizes are
  * copied there.  The call synchronises the stream ONCE, after the last step, to read a sticky device-side flag:

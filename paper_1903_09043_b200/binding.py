@@ -18,7 +18,7 @@ ARK_OK, ARK_EINVAL, ARK_ENOMEM, ARK_ECUDA, ARK_ENONFINITE = 0, -1, -2, -3, -4
 BC_PERIODIC, BC_REFLECTING, BC_FIXED_T_WALL, BC_FLUX_WALL = 0, 1, 2, 3
 
 EXPORTS = ["ark_workspace_bytes", "ark_create", "ark_set_state", "ark_get_state", "ark_set_state_host",
-           "ark_get_state_host", "ark_compute_dt", "ark_cfl_dt_static", "ark_cfl_dt_static_max_cells", "ark_step", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
+           "ark_get_state_host", "ark_compute_dt", "ark_cfl_dt_static", "ark_cfl_dt_static_max_cells", "ark_step", "ark_max_rate_device", "ark_step_device_dt", "ark_run", "ark_set_energy_form", "ark_potential_bytes", "ark_set_potential",
            "ark_halo_bytes", "ark_get_halo", "ark_set_halo", "ark_ke_spectrum_bins", "ark_ke_spectrum",
            "ark_diagnostics", "ark_debug_get_padded",
            "ark_step_kernel_timing", "ark_step_kernel_time", "ark_measure_fp64_peak", "ark_launch_count", "ark_destroy", "ark_last_error", "ark_version_string"]
@@ -61,6 +61,10 @@ def load():
     lib.ark_cfl_dt_static_max_cells.restype = C.c_size_t
     lib.ark_cfl_dt_static.argtypes = [ip, ip, ip, C.c_double, C.c_double, C.c_double, C.c_double] + [dp] * 5 + [C.c_double, dp, vp]
     lib.ark_cfl_dt_static.restype = ip
+    lib.ark_max_rate_device.argtypes = [vp, dp]
+    lib.ark_max_rate_device.restype = ip
+    lib.ark_step_device_dt.argtypes = [vp, dp]
+    lib.ark_step_device_dt.restype = ip
     lib.ark_step.argtypes = [vp, C.c_double]
     lib.ark_step.restype = ip
     lib.ark_diagnostics.argtypes = [vp, C.POINTER(C.c_double)]
@@ -305,6 +309,20 @@ class Solver:
 
     def step(self, dt):
         _check(self._lib.ark_step(self._h, float(dt)))
+
+    def _one_double(self, t, what):
+        if t.dtype != torch.float64 or t.numel() != 1 or t.device != self.workspace.device:
+            raise ValueError("%s must be a float64 CUDA tensor of 1 element on %s" % (what, self.workspace.device))
+        return C.c_void_p(t.data_ptr())
+
+    def max_rate_device(self, out):
+        """ark_max_rate_device: the maximum CFL rate of the current state -> out (1-element CUDA tensor), no host sync."""
+        _check(self._lib.ark_max_rate_device(self._h, self._one_double(out, "out")))
+        return out
+
+    def step_device_dt(self, dt):
+        """ark_step_device_dt: one step whose size is read from the 1-element CUDA tensor dt when the kernels run."""
+        _check(self._lib.ark_step_device_dt(self._h, self._one_double(dt, "dt")))
 
     def run(self, nsteps, cfl, want_dts=False):
         if want_dts:

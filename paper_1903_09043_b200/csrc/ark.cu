@@ -626,6 +626,24 @@ int ark_step(ark_solver* s, double dt) {
     return do_step(s, dt, nullptr);
 }
 
+// Device-side halves of {ark_compute_dt; ark_step} for time loops that must not wait for the host (see ark.h)
+int ark_max_rate_device(ark_solver* s, double* d_rate_out) {
+    if (!s || !d_rate_out) return fail(ARK_EINVAL, "ark_max_rate_device: NULL argument%s");
+    ARK_ON_DEVICE(s);
+    const int rc = reduce_rate(s, 1.0, nullptr);                 // result[0] = max rate of the current state
+    if (rc != ARK_OK) return rc;
+    ARK_CUDA(cudaMemcpyAsync(d_rate_out, s->result, sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return ARK_OK;
+}
+
+int ark_step_device_dt(ark_solver* s, const double* d_dt) {
+    if (!s || !d_dt) return fail(ARK_EINVAL, "ark_step_device_dt: NULL argument%s");
+    ARK_ON_DEVICE(s);
+    // the step kernels read a device-side step size from result[1] (where pass 2 of ark_run leaves it)
+    ARK_CUDA(cudaMemcpyAsync(s->result + 1, d_dt, sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return do_step(s, 0.0, s->result);
+}
+
 namespace {
 
 // one step of the device-side loop: dt = cfl / max rate (pass 2 on the rates of the current state), then the step

@@ -162,7 +162,10 @@ class SlabSolver:
             self.s.get_halo(0, self.send[0])
         if self.hi is not None:
             self.s.get_halo(1, self.send[1])
-        self.torch.cuda.current_stream(self.s.device).synchronize()      # the P2P ops run on the backend's own stream
+        if self.dist.get_backend() != "nccl":
+            # a backend that reads the buffers from the host side must see them finished; NCCL's P2P ops are enqueued
+            # behind the current stream (the solver's) and `wait()` makes that stream wait for them: no host stall
+            self.torch.cuda.current_stream(self.s.device).synchronize()
         exchange(self.dist, self.rank, self.world, self.periodic, self.send[0], self.send[1], self.recv[0], self.recv[1])
         if self.lo is not None:
             self.s.set_halo(0, self.recv[0])
@@ -172,6 +175,24 @@ class SlabSolver:
     def step(self, dt):
         self.halo_exchange()
         self.s.step(dt)
+
+    def step_cfl(self, cfl):
+        """One step of size cfl / (max over ALL ranks of the maximum CFL rate) with every number left on the device: the
+        local rate (ark_max_rate_device), a MAX all-reduce of one double, the division, the halo exchange and the step
+        (ark_step_device_dt) are all enqueued; the host never waits and never reads dt.  cfl / max rate is the same
+        double ark_compute_dt forms on the host (IEEE division).  Nothing checks the rate: call compute_dt now and then."""
+        t = self.torch
+        if not hasattr(self, "_rate"):
+            self._rate = t.empty(1, dtype=t.float64, device=self.s.device)
+            self._dt = t.empty(1, dtype=t.float64, device=self.s.device)
+            self._cfl = t.empty(1, dtype=t.float64, device=self.s.device)
+        self._cfl.fill_(float(cfl))
+        self.s.max_rate_device(self._rate)
+        if self.dist is not None and self.world > 1:
+            self.dist.all_reduce(self._rate, op=self.dist.ReduceOp.MAX)
+        t.div(self._cfl, self._rate, out=self._dt)
+        self.halo_exchange()
+        self.s.step_device_dt(self._dt)
 
     def bytes_per_exchange(self):
         """bytes this rank sends per step (what must cross NVLink)."""
@@ -205,7 +226,7 @@ class LocalSlabs:
     def compute_dt(self, cfl):
         return min(s.compute_dt(cfl) for s in self.solvers)
 
-    def step(self, dt):
+    def _exchange(self):
         if self.world > 1:
             halos = [(s.get_halo(0), s.get_halo(1)) for s in self.solvers]
             for r, s in enumerate(self.solvers):
@@ -214,8 +235,30 @@ class LocalSlabs:
                     s.set_halo(0, halos[lo][1])      # my low ghost planes = the high planes of the rank below
                 if hi is not None:
                     s.set_halo(1, halos[hi][0])
+
+    def step(self, dt):
+        self._exchange()
         for s in self.solvers:
             s.step(dt)
+
+    def step_cfl(self, cfl):
+        """The device-side loop of SlabSolver.step_cfl on one GPU: per-slab rates -> max -> dt = cfl / max, all in device
+        memory; no call of this method waits for the GPU or reads a number back."""
+        import torch
+        dev = self.solvers[0].device
+        if not hasattr(self, "_rates"):
+            self._rates = torch.empty(self.world, dtype=torch.float64, device=dev)
+            self._rate = torch.empty(1, dtype=torch.float64, device=dev)
+            self._dt = torch.empty(1, dtype=torch.float64, device=dev)
+            self._cfl = torch.empty(1, dtype=torch.float64, device=dev)
+        self._cfl.fill_(float(cfl))
+        for r, s in enumerate(self.solvers):
+            s.max_rate_device(self._rates[r:r + 1])
+        torch.amax(self._rates, dim=0, keepdim=True, out=self._rate)
+        torch.div(self._cfl, self._rate, out=self._dt)
+        self._exchange()
+        for s in self.solvers:
+            s.step_device_dt(self._dt)
 
     def close(self):
         for s in self.solvers:

@@ -765,6 +765,30 @@ def test_slab_decomposition_matches_the_undivided_domain(B, name):
     check_fields(ref, b, TOL, momentum_floor(prm, ref, dts), name)
 
 
+@pytest.mark.parametrize("name", sorted(SLAB))
+def test_slab_time_loop_without_host_round_trips(B, name):
+    """LocalSlabs.step_cfl: per-slab maximum rates (ark_max_rate_device), their maximum, dt = cfl / max and the steps
+    (ark_step_device_dt) all stay in device memory -- the loop a multi-GPU run needs to keep the host out of the way
+    (PAPER.md:291, :295).  Must give the state of the host loop {dt = min compute_dt; exchange; step(dt)} bit for bit:
+    the maximum does not depend on the split and cfl / max is an IEEE division on both sides."""
+    from paper_1903_09043_b200 import slab
+    (prm, U), world = SLAB[name]()
+    host = slab.LocalSlabs(B, prm, world)
+    host.set_state(to_dev(U))
+    devl = slab.LocalSlabs(B, prm, world)
+    devl.set_state(to_dev(U))
+    for _ in range(6):
+        host.step(host.compute_dt(0.4))
+        devl.step_cfl(0.4)
+    a, b = to_np(host.get_state()), to_np(devl.get_state())
+    dt_next = (host.compute_dt(0.4), devl.compute_dt(0.4))
+    host.close()
+    devl.close()
+    for f in range(5):
+        assert np.array_equal(a[f], b[f]), (name, f, float(np.abs(a[f] - b[f]).max()))
+    assert dt_next[0] == dt_next[1]
+
+
 def test_external_sides_are_validated(B):
     prm, _ = I.random_state(8, 8, 1, 1)
     with pytest.raises(B.ArkError):
